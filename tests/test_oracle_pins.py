@@ -1,0 +1,170 @@
+"""Pins of the CPU oracle against things the mathematics fixes (BASELINE.json invariants (i)-(v)).
+None of these re-types the oracle's own formula: each uses a closed form, an identity, a finite
+difference or explicit loops."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import exc_oracle as O
+from oracle import overlap as OV
+from paper_2605_10363_b200 import workloads as W
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def basis_of(wl):
+    return (wl.atom_xyz, wl.shell_atom, wl.shell_l, wl.shell_prim_off, wl.prim_alpha, wl.prim_coef)
+
+
+@pytest.fixture(scope="module")
+def water():
+    return W.named_config("cfg0")
+
+
+def test_component_order_and_count():
+    assert O.cart_components(1) == [(1, 0, 0), (0, 1, 0), (0, 0, 1)]
+    assert O.cart_components(2) == [(2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)]
+
+
+def test_overlap_diagonal_is_one(water):
+    S = OV.overlap_matrix(*basis_of(water))
+    assert np.max(np.abs(np.diag(S) - 1.0)) < 1e-14
+    assert np.max(np.abs(S - S.T)) == 0.0
+    # a textbook special case: two normalised s-Gaussians a,b at distance R:
+    # S = (2 sqrt(ab)/(a+b))^{3/2} exp(-ab/(a+b) R^2)
+    a, b, R = 1.5, 0.3, 1.7
+    xyz = np.array([[0.0, 0, 0], [0, 0, R]])
+    S2 = OV.overlap_matrix(xyz, [0, 1], [0, 0], [0, 1, 2], [a, b], [1.0, 1.0])
+    ref = (2 * math.sqrt(a * b) / (a + b)) ** 1.5 * math.exp(-a * b / (a + b) * R * R)
+    assert abs(S2[0, 1] - ref) < 1e-15
+
+
+def test_slater_closed_form_single_s_gaussian():
+    """Invariant (iv) + quadrature weights: one normalised s-Gaussian, alpha=1, n=2."""
+    alpha, n, ref = np.loadtxt(os.path.join(HERE, "golden", "slater_s_gaussian.txt"))
+    formula = -0.75 * (3 / math.pi) ** (1 / 3) * n ** (4 / 3) * (2 * alpha / math.pi) ** 2 * (3 * math.pi / (8 * alpha)) ** 1.5
+    assert abs(formula - ref) < 1e-10          # the fixture is the closed form
+    pts, w = W.atomic_grid(1.0)
+    basis = (np.zeros((1, 3)), np.array([0]), np.array([0]), np.array([0, 1]), np.array([alpha]), np.array([1.0]))
+    out = O.exc(basis, pts, w, np.array([[n]]), "lda")
+    assert abs(out["E"] - ref) < 2e-10 * abs(ref) + 1e-10
+    # number of electrons: exact angular rule for an s density
+    assert abs(float(np.sum(w * out["rho"])) - n) < 1e-9
+    # V is a 1x1 matrix: <chi| v |chi> = -(4/3) C_x n^{1/3} int rho1^{4/3}  (rho1 = density for n=1)
+    v_ref = (4.0 / 3.0) * ref / n
+    assert abs(out["V"][0, 0] - v_ref) < 1e-9
+
+
+def test_electron_count_equals_trace_DS(water):
+    """Invariant (i): int rho = Tr(D S).  1e-6 needs a verification grid (the 110-point equal-weight
+    angular rule limits the config grid to ~4e-4); the config grid must reach 1e-3."""
+    S = OV.overlap_matrix(*basis_of(water))
+    ne = float(np.sum(water.D * S))
+    out = O.exc(basis_of(water), water.grid_xyz, water.grid_w, water.D, "lda", want_v=False)
+    err_cfg = abs(float(np.sum(water.grid_w * out["rho"])) - ne) / abs(ne)
+    assert err_cfg < 1e-3
+    # verification grid: 80 radial x 16000 angular per atom
+    pts, w, owner = [], [], []
+    for ia, s in enumerate(water.symbols):
+        p, ww = W.atomic_grid({"H": 1.0, "O": 1.2}[s], n_rad=80, n_ang=16000)
+        pts.append(p + water.atom_xyz[ia]); w.append(ww); owner.append(np.full(len(ww), ia, np.int32))
+    pts = np.vstack(pts); w = np.concatenate(w); owner = np.concatenate(owner)
+    w = w * W.becke_weights(water.atom_xyz, pts, owner, backend="numpy")
+    rho = np.concatenate([O.rho_at_points(basis_of(water), pts[c:c + 65536], water.D)
+                          for c in range(0, len(pts), 65536)])
+    err_fine = abs(float(np.sum(w * rho)) - ne) / abs(ne)
+    assert err_fine < 1e-6
+    assert err_fine < err_cfg
+
+
+def test_v_symmetric_and_bruteforce(water):
+    """Invariants (ii) and (v) on single water (every 8th grid point for the Python loops)."""
+    sl = slice(0, None, 8)
+    pts, w = water.grid_xyz[sl], water.grid_w[sl]
+    out = O.exc(basis_of(water), pts, w, water.D, "lda", chunk=500)
+    V = out["V"]
+    assert np.max(np.abs(V - V.T)) <= 1e-13 * np.max(np.abs(V))
+    bf = O.brute_force_lda(basis_of(water), pts.tolist(), w.tolist(), water.D.tolist())
+    assert np.max(np.abs(bf["rho"] - out["rho"])) < 1e-12 * max(1.0, np.max(np.abs(out["rho"])))
+    assert abs(bf["E"] - out["E"]) < 1e-11 * abs(out["E"])
+    assert np.max(np.abs(bf["V"] - V)) < 1e-11 * np.max(np.abs(V))
+    # chunking must not matter
+    out2 = O.exc(basis_of(water), pts, w, water.D, "lda", chunk=100000)
+    assert np.max(np.abs(out2["V"] - V)) < 1e-12 * np.max(np.abs(V))
+
+
+@pytest.mark.parametrize("functional", ["lda", "gga"])
+def test_finite_difference_dE_dD_equals_V(water, functional):
+    """Invariant (iii): central differences of E_xc w.r.t. single elements D_{mu,nu} give V_{mu,nu}."""
+    basis = basis_of(water)
+    out = O.exc(basis, water.grid_xyz, water.grid_w, water.D, functional)
+    V = out["V"]
+    assert np.max(np.abs(V - V.T)) <= 1e-12 * np.max(np.abs(V))
+    h = 3e-5
+    scale = np.max(np.abs(V))
+    for (m, n) in [(0, 0), (2, 7), (7, 2), (3, 16), (12, 24), (20, 21)]:
+        Dp = water.D.copy(); Dp[m, n] += h
+        Dm = water.D.copy(); Dm[m, n] -= h
+        ep = O.exc(basis, water.grid_xyz, water.grid_w, Dp, functional, want_v=False)["E"]
+        em = O.exc(basis, water.grid_xyz, water.grid_w, Dm, functional, want_v=False)["E"]
+        fd = (ep - em) / (2 * h)
+        assert abs(fd - V[m, n]) < 1e-6 * scale, (functional, m, n, fd, V[m, n])
+
+
+def test_ao_gradient_matches_finite_difference(water):
+    basis = basis_of(water)
+    rng = np.random.default_rng(5)
+    pts = rng.uniform(-2.5, 2.5, size=(40, 3))
+    phi, dphi = O.ao_values(*basis, pts, deriv=True)
+    h = 1e-5
+    for c in range(3):
+        e = np.zeros(3); e[c] = h
+        fd = (O.ao_values(*basis, pts + e) - O.ao_values(*basis, pts - e)) / (2 * h)
+        assert np.max(np.abs(fd - dphi[c])) < 1e-8
+    # density gradient against the density at displaced points
+    rho, drho = O.rho_at_points(basis, pts, water.D, want_grad=True)
+    for c in range(3):
+        e = np.zeros(3); e[c] = h
+        fd = (O.rho_at_points(basis, pts + e, water.D) - O.rho_at_points(basis, pts - e, water.D)) / (2 * h)
+        assert np.max(np.abs(fd - drho[c])) < 1e-7
+
+
+def test_pbe_enhancement_limits():
+    rho = np.geomspace(1e-12, 50.0, 200)
+    e_s, v_s = O.slater(rho)
+    e0, v0, vs0 = O.pbe_x(rho, np.zeros_like(rho))
+    assert np.allclose(e0, e_s, rtol=1e-15, atol=0) and np.allclose(v0, v_s, rtol=1e-15, atol=0)   # F(0) = 1
+    e_m0, v_m0, vs_m0 = O.pbe_x(rho, rho ** 2, mu=0.0)                                            # mu = 0 -> Slater
+    assert np.allclose(e_m0, e_s, rtol=1e-15) and np.all(vs_m0 == 0.0)
+    e_inf, _, _ = O.pbe_x(rho, 1e40 * np.ones_like(rho))                                          # F(inf) = 1+kappa
+    assert np.allclose(e_inf, 1.804 * e_s, rtol=1e-12)
+    sig = np.geomspace(1e-10, 1e6, 200)
+    e, _, _ = O.pbe_x(rho, sig)
+    assert np.all(e <= e_s * (1 - 1e-14)) and np.all(e >= 1.804 * e_s * (1 + 1e-14))
+    # closed forms at one point: rho = 1, s^2 = 1  ->  sigma = 4 K_S
+    ks = (3 * math.pi ** 2) ** (2 / 3)
+    F = 1 + 0.804 - 0.804 / (1 + 0.21951 / 0.804)
+    e1, _, _ = O.pbe_x(np.array([1.0]), np.array([4 * ks]))
+    assert abs(e1[0] + 0.75 * (3 / math.pi) ** (1 / 3) * F) < 1e-15
+    # derivative consistency by finite differences in rho and sigma
+    r0, s0 = 0.37, 0.81
+    h = 1e-6
+    _, vr, vs = O.pbe_x(np.array([r0]), np.array([s0]))
+    fr = (O.pbe_x(np.array([r0 + h]), np.array([s0]))[0] - O.pbe_x(np.array([r0 - h]), np.array([s0]))[0]) / (2 * h)
+    fs = (O.pbe_x(np.array([r0]), np.array([s0 + h]))[0] - O.pbe_x(np.array([r0]), np.array([s0 - h]))[0]) / (2 * h)
+    assert abs(fr[0] - vr[0]) < 1e-8 and abs(fs[0] - vs[0]) < 1e-8
+    # the density guard (reading A9)
+    e_c, v_c = O.slater(np.array([0.0, -1e-25, 1e-21, 1e-19]))
+    assert np.all(e_c[:3] == 0) and np.all(v_c[:3] == 0) and e_c[3] < 0
+
+
+def test_sampled_entry_helpers_agree_with_dense(water):
+    basis = basis_of(water)
+    out = O.exc(basis, water.grid_xyz, water.grid_w, water.D, "gga")
+    pairs = [(0, 0), (3, 11), (24, 5)]
+    got = O.vxc_entries_from_wv(basis, water.grid_xyz, out["wv"], pairs, gga=True)
+    ref = np.array([out["V"][m, n] for m, n in pairs])
+    assert np.max(np.abs(got - ref)) < 1e-12
+    assert abs(O.exc_energy_from_rho(water.grid_w, out["rho"], out["drho"], "gga") - out["E"]) < 1e-13
