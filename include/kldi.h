@@ -1,0 +1,172 @@
+/* kldi.h — C ABI of the block-filtered Kohn-Sham EXC contraction library (B200 / sm_100a, FP64).
+ *
+ * Method: KerneLDI, arxiv/paper_2605_10363 (cited below as PAPER.md:<line>).  The library
+ * computes, on ONE GPU, the hot path of exchange-correlation (EXC) grid integration written as
+ * block-structured matrix products (Eq. 1-6):
+ *
+ *     Phi(g,mu) = chi_mu(r_g)                                  (Eq. 2)
+ *     X = Phi D,   rho(g) = sum_mu Phi(g,mu) X(g,mu)           (Eq. 4)
+ *     V = Phi^T diag(w v_xc) Phi                               (Eq. 3/5; b = 1)
+ *
+ * restricted to the block pairs that survive the block-level filter max|Phi_pq| >= eps
+ * (Eq. 11-14) and the executable-pair test a_pq*b_qr >= eps (Eq. 17-19,
+ * PAPER.md:195-216), stored in row- and column-oriented block-compressed layouts (BCS(R)/BCS(C),
+ * PAPER.md:176-191, 459-471).  A "grid block" p is 128 consecutive points of the Morton-sorted
+ * grid (Eq. 20); an "AO block" q is one shell (AO-shell partition).
+ *
+ * Conventions (all calls):
+ *   - "host" pointers are ordinary CPU memory; "dev" pointers are CUDA device memory on the
+ *     device that was current when the plan was created.  The caller owns every buffer it
+ *     passes; the library neither frees nor keeps caller pointers after a call returns.
+ *   - AO order at the boundary: shells in the order given, Cartesian components in the order
+ *     s | x,y,z | xx,xy,xz,yy,yz,zz; every component is individually normalised (<chi|chi> = 1
+ *     for an uncontracted shell with coef = 1).  Grid order: the caller's.  Every internal
+ *     permutation (Morton order of points, spatial order of atoms/shells) is undone before
+ *     results are written.
+ *   - Matrices are row-major, FP64.  D must be symmetric.
+ *   - All work is enqueued on the CUDA stream given to kldi_plan_create.  Calls are
+ *     asynchronous on that stream unless stated otherwise.
+ *   - Every function returns a kldi_status; on failure kldi_last_error() (thread-local) holds a
+ *     message, outputs are unspecified and the plan remains usable.  No exceptions, no aborts,
+ *     no CPU fallback: without a CUDA device every compute call returns KLDI_ECUDA.
+ */
+#ifndef KLDI_H_
+#define KLDI_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct kldi_plan kldi_plan; /* opaque; owns all of its device memory */
+
+typedef enum { KLDI_OK = 0, KLDI_EINVAL = -1, KLDI_ENOMEM = -2, KLDI_ECUDA = -3, KLDI_ESTATE = -4 } kldi_status;
+
+/* Exchange functionals, spin-restricted (b = 1):
+ *   KLDI_LDA_SLATER: e = -C_x rho^{4/3}, C_x = (3/4)(3/pi)^{1/3}
+ *   KLDI_GGA_PBEX  : e = -C_x rho^{4/3} F(s), F = 1 + kappa - kappa/(1 + mu s^2/kappa),
+ *                    s^2 = |grad rho|^2 / (4 (3 pi^2)^{2/3} rho^{8/3}), kappa = 0.804, mu = 0.21951
+ * Points with rho < 1e-20 contribute nothing (e = v = 0). */
+typedef enum { KLDI_LDA_SLATER = 0, KLDI_GGA_PBEX = 1 } kldi_functional;
+
+typedef struct {
+  int32_t n_atoms;
+  const double* xyz; /* host, [n_atoms][3], bohr */
+} kldi_atoms;
+
+/* Contracted Cartesian Gaussian shells:
+ *   chi(r) = sum_i coef[i] N_i (x-Ax)^a (y-Ay)^b (z-Az)^c exp(-alpha[i] |r-A|^2),  a+b+c = l,
+ *   N_i = (2 alpha_i/pi)^{3/4} (4 alpha_i)^{l/2} / sqrt((2a-1)!!(2b-1)!!(2c-1)!!).            */
+typedef struct {
+  int32_t n_shells;
+  const int32_t* atom;      /* host, [n_shells] index into kldi_atoms */
+  const int32_t* l;         /* host, [n_shells] 0, 1 or 2 (1, 3, 6 Cartesian components) */
+  const int32_t* nprim_off; /* host, [n_shells+1] offsets into alpha / coef */
+  const double* alpha;      /* host, exponents > 0 */
+  const double* coef;       /* host, coefficients of the NORMALISED primitives */
+} kldi_shells;
+
+typedef struct {
+  int64_t n_pts;
+  const double* xyz; /* host, [n_pts][3], bohr */
+  const double* w;   /* host, [n_pts] quadrature weights (may contain zeros) */
+} kldi_grid;
+
+/* Counters of a plan and of its most recent contraction calls. */
+typedef struct {
+  int64_t n_pts;            /* grid points given */
+  int64_t n_blocks;         /* grid blocks of 128 (last one padded with zero-weight points) */
+  int64_t n_blocks_nonempty;/* grid blocks that retain at least one AO block */
+  int32_t n_ao;
+  int32_t n_shells;         /* = number of AO blocks per grid block before filtering */
+  int32_t n_atoms;
+  int32_t want_gradients;
+  int64_t retained_blocks;  /* |S_A|: retained (grid block, AO block) pairs (Eq. 13) */
+  int64_t candidate_blocks; /* n_blocks * n_shells */
+  int64_t sum_k;            /* sum_p K_p, K_p = retained AO columns of grid block p (unpadded) */
+  int64_t sum_k_pad;        /* same with each K_p padded to a multiple of 8 */
+  int64_t max_k;            /* max_p K_p */
+  int64_t phi_bytes;        /* device bytes of the stored Phi (and gradient) tiles */
+  int64_t workspace_bytes;  /* other device bytes owned by the plan */
+  double flops_rho_useful;  /* sum_p 2*128*K_p^2            (retained-block FLOPs of one rho build) */
+  double flops_rho_exec;    /* FLOPs the rho kernel issues (padding and symmetry accounted) */
+  double flops_v_useful;    /* LDA: sum_p 128*K_p*(K_p+1) (q<=r only); GGA: sum_p 2*128*K_p^2 */
+  double flops_v_exec;      /* FLOPs the V kernel issues (whole tiles, padded) */
+  double flops_dense;       /* 2*n_pts*n_ao^2 : one dense product */
+  double plan_seconds;      /* wall time of kldi_plan_create */
+  double eps;
+} kldi_stats;
+
+/* Once per geometry: Morton reorder of the grid into blocks of 128 (Eq. 20), spatial
+ * order of atoms and the AO-shell partition, AO evaluation on candidate (grid block, shell) tiles,
+ * block-max filter (keep iff max|chi| >= eps, Eq. 12; with want_gradients the max also runs over the
+ * three gradient components), BCS(R)/BCS(C) layouts, task lists.  eps <= 0 retains every block
+ * (dense; for tests).  want_gradients: 0 = values only (LDA), 1 = values + gradients (GGA).
+ * cuda_stream: a cudaStream_t (NULL = default stream) used by every later call on this plan.
+ * Synchronises the stream before returning.  *out is NULL on failure. */
+kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid,
+                             double eps, int want_gradients, void* cuda_stream, kldi_plan** out);
+kldi_status kldi_plan_destroy(kldi_plan* plan);
+kldi_status kldi_plan_stats(const kldi_plan* plan, kldi_stats* out);
+
+/* rho[g] = sum_{mu,nu} D[mu][nu] chi_mu(r_g) chi_nu(r_g) over executable block pairs
+ * (Eq. 4/18); if drho != NULL (plan needs want_gradients) also drho[c][g] = d rho / d r_c.
+ *   D    dev [n_ao][n_ao]   rho  dev [n_pts]   drho  dev [3][n_pts] or NULL                        */
+kldi_status kldi_eval_rho(kldi_plan* plan, const double* D, double* rho, double* drho);
+
+/* V = Phi^T diag(wv) Phi over retained block pairs (Eq. 5/16), wv = w*v_xc supplied by the caller.
+ * With gga != 0 (plan needs want_gradients): wv is [4][n_pts] with wv[0] = w v_rho,
+ * wv[1+c] = 2 w v_sigma d_c rho, and V = B + B^T, B = Phi^T (1/2 wv0 Phi + sum_c wv_c d_c Phi).
+ *   wv  dev [n_pts] or [4][n_pts]     V  dev [n_ao][n_ao], overwritten, exactly symmetric          */
+kldi_status kldi_build_vxc(kldi_plan* plan, const double* wv, int gga, double* V);
+
+/* The LDA/GGA driver: rho (and grad rho) -> functional -> E_xc = sum_g w_g e_g and V.
+ *   D dev [n_ao][n_ao];  Exc HOST, one value, valid on return (the call synchronises the stream);
+ *   V dev [n_ao][n_ao] or NULL (energy only).                                                    */
+kldi_status kldi_exc(kldi_plan* plan, const double* D, kldi_functional f, double* Exc, double* V);
+
+/* Same as kldi_exc with HOST buffers: copies D to the device, runs, copies V back (end-to-end
+ * timing; D_host/V_host should be page-locked for full PCIe speed but need not be). */
+kldi_status kldi_exc_host(kldi_plan* plan, const double* D_host, kldi_functional f, double* Exc,
+                          double* V_host);
+
+/* Device times (ms) of the stages of the most recent kldi_exc / kldi_eval_rho / kldi_build_vxc on
+ * this plan, measured with CUDA events on the plan's stream.  Synchronises.  out[8] HOST:
+ *   [0] D permute + block maxima  [1] rho contraction  [2] functional + energy  [3] wv gather / Z build
+ *   [4] V contraction  [5] V finalise  [6] total  [7] reserved                                   */
+kldi_status kldi_last_timings(kldi_plan* plan, double* out);
+
+/* Inspection of the plan's index structures (tests of Eq. 20 / BCS invariants).  Copies array
+ * `which` to host memory `buf` (capacity cap_bytes), writes the byte size to *need_bytes; with
+ * buf == NULL only the size is returned.  Arrays (int32 unless noted):
+ *   0 perm_g       [n_blocks*128] caller index of sorted point i, -1 for padding
+ *   1 row_ptr      [n_blocks+1]   BCS(R): retained AO blocks of grid block p are col_idx[row_ptr[p]..)
+ *   2 col_idx      [retained]     AO block (shell, in the plan's spatial shell order), increasing
+ *   3 col_ptr      [n_shells+1]   BCS(C): grid blocks retaining AO block q are row_idx[col_ptr[q]..)
+ *   4 row_idx      [retained]     grid block, increasing
+ *   5 pos          [retained]     BCS(C) -> BCS(R) position of the same block
+ *   6 shell_perm   [n_shells]     caller shell index of plan shell q
+ *   7 ao_perm      [n_ao]         caller AO index of plan AO i
+ *   8 morton_keys  [n_blocks*128] uint64, sorted keys (padding = 2^63)
+ *   9 block_amax   [retained]     float64, a_pq = max|Phi_pq| in BCS(R) order
+ *  10 panel_off    [n_blocks+1]   int64, first packed column of grid block p in the Phi store
+ *  11 blk_col0     [retained]     packed column (within its panel) where the block starts       */
+kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_t cap_bytes,
+                             int64_t* need_bytes);
+
+/* Copies the stored Phi tile (c = 0) or gradient tile (c = 1..3) of BCS(R) entry `entry` to host
+ * memory: out[k][128] for the block's columns k (column-major tile, 128 sorted points each). */
+kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, double* out,
+                                  int64_t cap_bytes, int32_t* width);
+
+/* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`
+ * iterations; returns achieved TFLOP/s (device-timed) in *tflops.  kind 0 = DMMA, 1 = DFMA. */
+kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);
+
+const char* kldi_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KLDI_H_ */

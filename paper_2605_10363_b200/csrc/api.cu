@@ -1,0 +1,369 @@
+// C ABI entry points of libkldi (declared in include/kldi.h).
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "kldi_internal.h"
+#include "ptx.cuh"
+
+namespace kldi {
+static thread_local char g_err[512] = "";
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+// ------------------------------------------------------------------ FP64 pipe microbenchmark
+__global__ void __launch_bounds__(256) k_peak_dmma(int iters, double* sink) {
+  double c[16][2];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) c[i][0] = c[i][1] = 0.0;
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) dmma884(c[i][0], c[i][1], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+  if (s == 123.456) sink[0] = s;
+}
+__global__ void __launch_bounds__(256) k_peak_dfma(int iters, double* sink) {
+  double c[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) c[i] = i;
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = fma(c[i], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i];
+  if (s == 123.456) sink[0] = s;
+}
+}  // namespace kldi
+
+using namespace kldi;
+
+extern "C" {
+
+const char* kldi_last_error(void) { return g_err; }
+
+kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid, double eps,
+                             int want_gradients, void* cuda_stream, kldi_plan** out) {
+  if (out) *out = nullptr;
+  if (!atoms || !shells || !grid || !out || !atoms->xyz || !shells->atom || !shells->l || !shells->nprim_off ||
+      !shells->alpha || !shells->coef || !grid->xyz || !grid->w || atoms->n_atoms <= 0 || shells->n_shells <= 0 ||
+      grid->n_pts <= 0 || !(eps == eps)) {
+    set_error("kldi_plan_create: null or empty argument");
+    return KLDI_EINVAL;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    set_error("kldi_plan_create: no CUDA device (this library has no CPU path)");
+    return KLDI_ECUDA;
+  }
+  kldi_plan* P = new (std::nothrow) kldi_plan();
+  if (!P) return KLDI_ENOMEM;
+  P->stream = (cudaStream_t)cuda_stream;
+  P->eps = eps;
+  P->want_grad = want_gradients ? 1 : 0;
+  cudaGetDevice(&P->device);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, P->device) != cudaSuccess || prop.major < 10) {
+    set_error("kldi_plan_create: device is not sm_100+ (found sm_%d%d)", prop.major, prop.minor);
+    delete P;
+    return KLDI_ECUDA;
+  }
+  P->n_sm = prop.multiProcessorCount;
+  kldi_status rc = plan_build(P, atoms, shells, grid);
+  if (rc != KLDI_OK) {
+    plan_free(P);
+    delete P;
+    return rc;
+  }
+  if (P->stats.max_k >= 32760) {
+    set_error("kldi_plan_create: a grid block retains %lld AO columns (limit 32759)", (long long)P->stats.max_k);
+    plan_free(P);
+    delete P;
+    return KLDI_EINVAL;
+  }
+  // FLOPs the kernels issue (whole DMMA tiles)
+  double fr = 0, fv = 0;
+  for (int64_t p = 0; p < P->n_blocks; ++p) {
+    const double k8 = (double)(P->h_panel_off[p + 1] - P->h_panel_off[p]);
+    fr += 2.0 * GB * k8 * k8;
+    const int nt = ((int)k8 + 63) / 64;
+    if (nt) {
+      const int W = ((((int)k8 + nt - 1) / nt) + 7) & ~7;
+      for (int i = 0; i < nt; ++i)
+        for (int j = P->want_grad ? 0 : i; j < nt; ++j)
+          fv += 2.0 * GB * std::min(W, (int)k8 - i * W) * (double)std::min(W, (int)k8 - j * W);
+    }
+  }
+  P->stats.flops_rho_exec = fr;
+  P->stats.flops_v_exec = fv;
+  *out = P;
+  return KLDI_OK;
+}
+
+kldi_status kldi_plan_destroy(kldi_plan* P) {
+  if (!P) return KLDI_OK;
+  plan_free(P);
+  delete P;
+  return KLDI_OK;
+}
+
+kldi_status kldi_plan_stats(const kldi_plan* P, kldi_stats* out) {
+  if (!P || !out) {
+    set_error("kldi_plan_stats: null argument");
+    return KLDI_EINVAL;
+  }
+  *out = P->stats;
+  return KLDI_OK;
+}
+
+#define EV(i) KLDI_CUDA(cudaEventRecord(P->ev[i], P->stream))
+
+kldi_status kldi_eval_rho(kldi_plan* P, const double* D, double* rho, double* drho) {
+  if (!P || !D || !rho) {
+    set_error("kldi_eval_rho: null argument");
+    return KLDI_EINVAL;
+  }
+  if (drho && !P->want_grad) {
+    set_error("kldi_eval_rho: gradients requested from a plan created with want_gradients = 0");
+    return KLDI_ESTATE;
+  }
+  kldi_status rc;
+  P->have_timings = false;
+  EV(0);
+  if ((rc = launch_permute_D(P, D)) != KLDI_OK) return rc;
+  EV(1);
+  if ((rc = launch_rho(P, drho != nullptr)) != KLDI_OK) return rc;
+  EV(2);
+  if ((rc = launch_unpermute_rho(P, rho, drho)) != KLDI_OK) return rc;
+  for (int i = 3; i < 7; ++i) EV(i);
+  P->have_timings = true;
+  return KLDI_OK;
+}
+
+kldi_status kldi_build_vxc(kldi_plan* P, const double* wv, int gga, double* V) {
+  if (!P || !wv || !V) {
+    set_error("kldi_build_vxc: null argument");
+    return KLDI_EINVAL;
+  }
+  if (gga && !P->want_grad) {
+    set_error("kldi_build_vxc: GGA form requested from a plan created with want_gradients = 0");
+    return KLDI_ESTATE;
+  }
+  kldi_status rc;
+  P->have_timings = false;
+  for (int i = 0; i < 4; ++i) EV(i);
+  if ((rc = launch_gather_wv(P, wv, gga != 0)) != KLDI_OK) return rc;
+  EV(4);
+  if ((rc = launch_vxc(P, gga != 0)) != KLDI_OK) return rc;
+  EV(5);
+  if ((rc = launch_finalise_V(P, gga != 0, V)) != KLDI_OK) return rc;
+  EV(6);
+  P->have_timings = true;
+  return KLDI_OK;
+}
+
+static kldi_status exc_enqueue(kldi_plan* P, const double* D, kldi_functional f, double* V) {
+  const bool gga = (f == KLDI_GGA_PBEX);
+  kldi_status rc;
+  P->have_timings = false;
+  EV(0);
+  if ((rc = launch_permute_D(P, D)) != KLDI_OK) return rc;
+  EV(1);
+  if ((rc = launch_rho(P, gga)) != KLDI_OK) return rc;
+  EV(2);
+  if ((rc = launch_xc(P, f)) != KLDI_OK) return rc;
+  EV(3);
+  EV(4);
+  if (V) {
+    if ((rc = launch_vxc(P, gga)) != KLDI_OK) return rc;
+    EV(5);
+    if ((rc = launch_finalise_V(P, gga, V)) != KLDI_OK) return rc;
+  } else {
+    EV(5);
+  }
+  EV(6);
+  KLDI_CUDA(cudaMemcpyAsync(P->h_E, P->d_E, sizeof(double), cudaMemcpyDeviceToHost, P->stream));
+  P->have_timings = true;
+  return KLDI_OK;
+}
+
+kldi_status kldi_exc(kldi_plan* P, const double* D, kldi_functional f, double* Exc, double* V) {
+  if (!P || !D || !Exc || (f != KLDI_LDA_SLATER && f != KLDI_GGA_PBEX)) {
+    set_error("kldi_exc: null argument or unknown functional");
+    return KLDI_EINVAL;
+  }
+  if (f == KLDI_GGA_PBEX && !P->want_grad) {
+    set_error("kldi_exc: GGA functional needs a plan created with want_gradients = 1");
+    return KLDI_ESTATE;
+  }
+  kldi_status rc = exc_enqueue(P, D, f, V);
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));
+  *Exc = *P->h_E;
+  return KLDI_OK;
+}
+
+kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f, double* Exc, double* V_host) {
+  if (!P || !D_host || !Exc || (f != KLDI_LDA_SLATER && f != KLDI_GGA_PBEX)) {
+    set_error("kldi_exc_host: null argument or unknown functional");
+    return KLDI_EINVAL;
+  }
+  if (f == KLDI_GGA_PBEX && !P->want_grad) {
+    set_error("kldi_exc_host: GGA functional needs a plan created with want_gradients = 1");
+    return KLDI_ESTATE;
+  }
+  const size_t nn = sizeof(double) * (size_t)P->n_ao * P->n_ao;
+  if (!P->d_stage_host) KLDI_CUDA(cudaMalloc(&P->d_stage_host, 2 * nn));
+  double* dD = P->d_stage_host;
+  double* dV = V_host ? P->d_stage_host + (size_t)P->n_ao * P->n_ao : nullptr;
+  KLDI_CUDA(cudaMemcpyAsync(dD, D_host, nn, cudaMemcpyHostToDevice, P->stream));
+  kldi_status rc = exc_enqueue(P, dD, f, dV);
+  if (rc != KLDI_OK) return rc;
+  if (V_host) KLDI_CUDA(cudaMemcpyAsync(V_host, dV, nn, cudaMemcpyDeviceToHost, P->stream));
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));
+  *Exc = *P->h_E;
+  return KLDI_OK;
+}
+
+kldi_status kldi_last_timings(kldi_plan* P, double* out) {
+  if (!P || !out) {
+    set_error("kldi_last_timings: null argument");
+    return KLDI_EINVAL;
+  }
+  if (!P->have_timings) {
+    set_error("kldi_last_timings: no completed call on this plan");
+    return KLDI_ESTATE;
+  }
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));
+  for (int i = 0; i < 6; ++i) {
+    float ms = 0.f;
+    KLDI_CUDA(cudaEventElapsedTime(&ms, P->ev[i], P->ev[i + 1]));
+    out[i] = ms;
+  }
+  float ms = 0.f;
+  KLDI_CUDA(cudaEventElapsedTime(&ms, P->ev[0], P->ev[6]));
+  out[6] = ms;
+  out[7] = 0.0;
+  return KLDI_OK;
+}
+
+kldi_status kldi_plan_export(const kldi_plan* P, int which, void* buf, int64_t cap, int64_t* need) {
+  if (!P || !need) {
+    set_error("kldi_plan_export: null argument");
+    return KLDI_EINVAL;
+  }
+  const void* hsrc = nullptr;
+  const void* dsrc = nullptr;
+  int64_t bytes = 0;
+  switch (which) {
+    case 0: dsrc = P->d_perm_g; bytes = 4 * P->n_pad; break;
+    case 1: hsrc = P->h_row_ptr.data(); bytes = 4 * (int64_t)P->h_row_ptr.size(); break;
+    case 2: hsrc = P->h_col_idx.data(); bytes = 4 * (int64_t)P->h_col_idx.size(); break;
+    case 3: hsrc = P->h_col_ptr.data(); bytes = 4 * (int64_t)P->h_col_ptr.size(); break;
+    case 4: hsrc = P->h_row_idx.data(); bytes = 4 * (int64_t)P->h_row_idx.size(); break;
+    case 5: hsrc = P->h_pos.data(); bytes = 4 * (int64_t)P->h_pos.size(); break;
+    case 6: hsrc = P->h_shell_perm.data(); bytes = 4 * (int64_t)P->h_shell_perm.size(); break;
+    case 7: hsrc = P->h_ao_perm.data(); bytes = 4 * (int64_t)P->h_ao_perm.size(); break;
+    case 8: dsrc = P->d_keys; bytes = 8 * P->n_pad; break;
+    case 9: dsrc = P->d_blk_amax; bytes = 8 * (int64_t)P->h_col_idx.size(); break;
+    case 10: hsrc = P->h_panel_off.data(); bytes = 8 * (int64_t)P->h_panel_off.size(); break;
+    case 11: hsrc = P->h_blk_col0.data(); bytes = 4 * (int64_t)P->h_blk_col0.size(); break;
+    default: set_error("kldi_plan_export: unknown array %d", which); return KLDI_EINVAL;
+  }
+  *need = bytes;
+  if (!buf) return KLDI_OK;
+  if (cap < bytes) {
+    set_error("kldi_plan_export: buffer too small (%lld < %lld)", (long long)cap, (long long)bytes);
+    return KLDI_EINVAL;
+  }
+  if (hsrc) {
+    memcpy(buf, hsrc, (size_t)bytes);
+  } else {
+    KLDI_CUDA(cudaStreamSynchronize(P->stream));
+    KLDI_CUDA(cudaMemcpy(buf, dsrc, (size_t)bytes, cudaMemcpyDeviceToHost));
+  }
+  return KLDI_OK;
+}
+
+kldi_status kldi_plan_export_tile(const kldi_plan* P, int64_t entry, int c, double* out, int64_t cap, int32_t* width) {
+  if (!P || !out || !width || entry < 0 || entry >= (int64_t)P->h_col_idx.size() || c < 0 || c > 3 ||
+      (c > 0 && !P->want_grad)) {
+    set_error("kldi_plan_export_tile: bad argument");
+    return KLDI_EINVAL;
+  }
+  // grid block of the entry: binary search in row_ptr
+  int64_t lo = 0, hi = P->n_blocks;
+  while (hi - lo > 1) {
+    const int64_t mid = (lo + hi) / 2;
+    if (P->h_row_ptr[mid] <= entry) lo = mid; else hi = mid;
+  }
+  const int64_t p = lo;
+  const int32_t c0 = P->h_blk_col0[entry];
+  const int32_t c1 = (entry + 1 < P->h_row_ptr[p + 1]) ? P->h_blk_col0[entry + 1] : -1;
+  int32_t w;
+  if (c1 >= 0) {
+    w = c1 - c0;
+  } else {  // last block of the row: width from the shell table is not on the host; use K_p
+    int32_t kp = 0;
+    KLDI_CUDA(cudaMemcpy(&kp, P->d_kp + p, sizeof(int32_t), cudaMemcpyDeviceToHost));
+    w = kp - c0;
+  }
+  *width = w;
+  const int64_t bytes = (int64_t)w * GB * 8;
+  if (cap < bytes) {
+    set_error("kldi_plan_export_tile: buffer too small");
+    return KLDI_EINVAL;
+  }
+  const double* src = (c == 0 ? P->d_phi : P->d_dphi[c - 1]) + (P->h_panel_off[p] + c0) * GB;
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));
+  KLDI_CUDA(cudaMemcpy(out, src, (size_t)bytes, cudaMemcpyDeviceToHost));
+  return KLDI_OK;
+}
+
+kldi_status kldi_fp64_peak(int kind, int iters, double* tflops) {
+  if (!tflops || iters <= 0) {
+    set_error("kldi_fp64_peak: bad argument");
+    return KLDI_EINVAL;
+  }
+  int dev = 0, nsm = 0;
+  KLDI_CUDA(cudaGetDevice(&dev));
+  KLDI_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  double* sink = nullptr;
+  KLDI_CUDA(cudaMalloc(&sink, 8));
+  cudaEvent_t e0, e1;
+  KLDI_CUDA(cudaEventCreate(&e0));
+  KLDI_CUDA(cudaEventCreate(&e1));
+  const int grid = nsm * 4;
+  for (int rep = 0; rep < 2; ++rep) {  // first pass warms up
+    KLDI_CUDA(cudaEventRecord(e0));
+    if (kind == 0)
+      k_peak_dmma<<<grid, 256>>>(iters, sink);
+    else
+      k_peak_dfma<<<grid, 256>>>(iters, sink);
+    KLDI_CUDA(cudaEventRecord(e1));
+    KLDI_CUDA(cudaEventSynchronize(e1));
+  }
+  float ms = 0.f;
+  KLDI_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+  const double per_thread_block = (kind == 0) ? 8.0 * 16 * 2 * 8 * 8 * 4 : 256.0 * 16 * 2;  // flops per CTA per iter
+  *tflops = per_thread_block * iters * grid / (ms * 1e-3) / 1e12;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  return KLDI_OK;
+}
+
+}  // extern "C"

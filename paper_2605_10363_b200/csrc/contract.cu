@@ -1,0 +1,577 @@
+// Per-evaluation kernels of libkldi (the hot path).  sm_100a, FP64.
+//   H1 k_permute_D   — D in plan AO order
+//   H2 k_rho         — X_p = Phi_p D[L(p),L(p)], rho_p = rowsum(Phi_p o X_p) (Eq. 4/18)
+//   H3 k_xc          — Slater / PBE-x per point, wv = w v, deterministic energy reduction (Eq. 1/3)
+//   H4 k_vxc         — G_p = Phi_p^T diag(wv_p) Phi_p scattered into V (Eq. 5/16)
+//   H5 k_finalise_V  — mirror / symmetrise, back to caller AO order
+// H2 and H4 are persistent, warp-specialised kernels: one producer warp pulls grid-block tasks
+// from an atomic ticket (the paper's pull-based pool, on-device) and streams
+// operand tiles through an mbarrier ring with bulk-async copies (TMA engine) and 8-byte cp.async;
+// eight consumer warps issue FP64 tensor-core MMAs (DMMA.8x8x4) on register accumulators.
+#include <cstdio>
+
+#include "kldi_internal.h"
+#include "ptx.cuh"
+
+namespace kldi {
+
+constexpr int LD = GB + 4;  // padded smem leading dimension of a 128-row column: conflict-free 8-B fragments
+
+// ===================================================================================== H1
+__global__ void k_permute_D(const double* __restrict__ D, const int32_t* __restrict__ ao_perm, int n,
+                            double* __restrict__ Dp) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j < n) Dp[(int64_t)i * n + j] = D[(int64_t)ao_perm[i] * n + ao_perm[j]];
+}
+
+// ===================================================================================== H2
+namespace rho {
+constexpr int NST = 3;                    // ring stages
+constexpr int KC = 32;                    // packed columns (K) per stage
+constexpr int NT = 128;                   // max N-tile width
+constexpr int PHI_BYTES = KC * LD * 8;    // 33,792
+constexpr int D_BYTES = KC * (NT + 4) * 8;  // 33,792
+constexpr int STAGE_BYTES = PHI_BYTES + D_BYTES;
+constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
+enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
+}  // namespace rho
+
+template <bool FULL>
+__device__ __forceinline__ void rho_ksteps(double (&acc)[2][16][2], const double* __restrict__ ps,
+                                           const double* __restrict__ ds, int nks, int nW) {
+  for (int ks = 0; ks < nks; ++ks) {
+    const double a0 = ps[ks * 4 * LD], a1 = ps[ks * 4 * LD + 8];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      if (FULL || j < nW) {
+        const double b = ds[ks * 4 * (rho::NT + 4) + 8 * j];
+        dmma884(acc[0][j][0], acc[0][j][1], a0, b);
+        dmma884(acc[1][j][0], acc[1][j][1], a1, b);
+      }
+    }
+  }
+}
+
+template <bool GGA>
+__global__ void __launch_bounds__(288, 1)
+    k_rho(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
+          const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
+          const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
+          const double* __restrict__ dphi2, const double* __restrict__ Dp, int n_ao, double* __restrict__ rho_s,
+          double* __restrict__ drho_s, int64_t n_pad) {
+  using namespace rho;
+  extern __shared__ __align__(128) unsigned char smem[];
+  int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
+  const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);  // full[s] at +8s, empty[s] at +8(NST+s)
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(bar0 + 8 * s, 33);         // producer lane 0 (expect_tx) + 32 cp.async completions
+      mbar_init(bar0 + 8 * (NST + s), 8);  // one arrive per consumer warp
+    }
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  if (warp == 8) {
+    // ------------------------------------------------------------------ producer warp
+    int s = 0;
+    uint32_t ph = 0;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(ticket, 1);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t >= n_tasks) break;
+      const int p = tasks[t];
+      const int K8 = (kp[p] + 7) & ~7;
+      const int64_t base = panel_off[p];
+      const int ntile = (K8 + NT - 1) / NT;
+      const int W = (((K8 + ntile - 1) / ntile) + 7) & ~7;
+      for (int jt = 0; jt < ntile; ++jt) {
+        const int n0 = jt * W, Wj = min(W, K8 - n0);
+        int cn[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) cn[c] = (lane + 32 * c < Wj) ? colidx[base + n0 + lane + 32 * c] : -1;
+        for (int k0 = 0; k0 < K8; k0 += KC) {
+          const int kc = min(KC, K8 - k0);
+          mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+          const int rowidx = (lane < kc) ? colidx[base + k0 + lane] : 0;
+          const uint32_t full = bar0 + 8 * s;
+          if (lane == 0) {
+            int fl = 0;
+            if (k0 == 0) fl |= F_FIRST;
+            if (k0 + KC >= K8) {
+              fl |= F_LAST_TILE;
+              if (jt == ntile - 1) fl |= F_LAST_PANEL;
+            }
+            hdr[4 * s + 0] = p;
+            hdr[4 * s + 1] = n0;
+            hdr[4 * s + 2] = (kc >> 2) | ((Wj >> 3) << 8) | (fl << 16);
+            mbar_arrive_expect_tx(full, (uint32_t)kc * (GB * 8));
+          }
+          __syncwarp();
+          const uint32_t sphi = smem_u32(smem + s * STAGE_BYTES);
+          const uint32_t sd = sphi + PHI_BYTES;
+          if (lane < kc) bulk_g2s(sphi + lane * (LD * 8), phi + (base + k0 + lane) * GB, GB * 8, full);
+          for (int r = 0; r < kc; ++r) {
+            const int row = __shfl_sync(0xffffffffu, rowidx, r);
+            const double* drow = Dp + (int64_t)row * n_ao;
+            const uint32_t dst = sd + (r * (NT + 4) + lane) * 8;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+              if (cn[c] >= 0) cp_async8(dst + c * 256, drow + cn[c]);
+          }
+          cp_async_mbar_arrive_noinc(full);
+          if (++s == NST) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+    mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+    if (lane == 0) {
+      hdr[4 * s + 2] = F_DONE << 16;
+      mbar_arrive(bar0 + 8 * s);
+    }
+    cp_async_mbar_arrive_noinc(bar0 + 8 * s);
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumer warps (16 rows each)
+  double acc[2][16][2];
+  double rs[GGA ? 4 : 1][2];
+#pragma unroll
+  for (int c = 0; c < (GGA ? 4 : 1); ++c) rs[c][0] = rs[c][1] = 0.0;
+  int s = 0;
+  uint32_t ph = 0;
+  const int q4 = lane >> 2, r4 = lane & 3;
+  for (;;) {
+    mbar_wait(bar0 + 8 * s, ph);
+    const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
+    const int fl = h2 >> 16;
+    if (fl & F_DONE) break;
+    const int nks = h2 & 0xff, nW = (h2 >> 8) & 0xff;
+    if (fl & F_FIRST) {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
+    }
+    const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 16 * warp + q4;
+    const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
+    if (nW == 16)
+      rho_ksteps<true>(acc, ps, ds, nks, nW);
+    else
+      rho_ksteps<false>(acc, ps, ds, nks, nW);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    if (++s == NST) { s = 0; ph ^= 1; }
+
+    if (fl & F_LAST_TILE) {
+      // epilogue: rho_p += rowsum(Phi_p[:, tile] o X[:, tile]); GGA: d_c rho_p += 2 rowsum(d_c Phi o X)
+      const int64_t off = (panel_off[p] + n0 + 2 * r4) * GB + 16 * warp + q4;
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        if (j < nW) {
+          const int64_t o = off + (int64_t)j * 8 * GB;
+          rs[0][0] += acc[0][j][0] * phi[o] + acc[0][j][1] * phi[o + GB];
+          rs[0][1] += acc[1][j][0] * phi[o + 8] + acc[1][j][1] * phi[o + GB + 8];
+          if (GGA) {
+            rs[1][0] += acc[0][j][0] * dphi0[o] + acc[0][j][1] * dphi0[o + GB];
+            rs[1][1] += acc[1][j][0] * dphi0[o + 8] + acc[1][j][1] * dphi0[o + GB + 8];
+            rs[2][0] += acc[0][j][0] * dphi1[o] + acc[0][j][1] * dphi1[o + GB];
+            rs[2][1] += acc[1][j][0] * dphi1[o + 8] + acc[1][j][1] * dphi1[o + GB + 8];
+            rs[3][0] += acc[0][j][0] * dphi2[o] + acc[0][j][1] * dphi2[o + GB];
+            rs[3][1] += acc[1][j][0] * dphi2[o + 8] + acc[1][j][1] * dphi2[o + GB + 8];
+          }
+        }
+      }
+      if (fl & F_LAST_PANEL) {
+#pragma unroll
+        for (int c = 0; c < (GGA ? 4 : 1); ++c)
+#pragma unroll
+          for (int mi = 0; mi < 2; ++mi) {
+            double v = rs[c][mi];
+            v += __shfl_xor_sync(0xffffffffu, v, 1);
+            v += __shfl_xor_sync(0xffffffffu, v, 2);
+            if (r4 == 0) {
+              const int64_t g = (int64_t)p * GB + 16 * warp + 8 * mi + q4;
+              if (c == 0)
+                rho_s[g] = v;
+              else
+                drho_s[(int64_t)(c - 1) * n_pad + g] = 2.0 * v;
+            }
+            rs[c][mi] = 0.0;
+          }
+      }
+    }
+  }
+}
+
+// ===================================================================================== H3
+constexpr double C_X = 0.73855876638202240588;    // (3/4)(3/pi)^{1/3}
+constexpr double K_S = 9.5707800006273016908;     // (3 pi^2)^{2/3}
+constexpr double PBE_KAPPA = 0.804, PBE_MU = 0.21951, RHO_CUT = 1e-20;
+
+template <bool GGA>
+__global__ void __launch_bounds__(256) k_xc(int64_t n_pad, const double* __restrict__ rho_s,
+                                            const double* __restrict__ drho_s, const double* __restrict__ gw,
+                                            double* __restrict__ wv_s, double* __restrict__ epart) {
+  __shared__ double red[256];
+  const int64_t g = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  double we = 0.0;
+  if (g < n_pad) {
+    const double r = rho_s[g], w = gw[g];
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
+    if (r >= RHO_CUT) {
+      const double c = cbrt(r);
+      if (!GGA) {
+        we = w * (-C_X * r * c);
+        v0 = w * (-(4.0 / 3.0) * C_X * c);
+      } else {
+        const double dx = drho_s[g], dy = drho_s[n_pad + g], dz = drho_s[2 * n_pad + g];
+        const double sigma = dx * dx + dy * dy + dz * dz;
+        const double r43 = r * c;
+        const double s2 = sigma / (4.0 * K_S * r43 * r43);
+        const double den = 1.0 + PBE_MU * s2 / PBE_KAPPA;
+        const double F = 1.0 + PBE_KAPPA - PBE_KAPPA / den;
+        const double Fp = PBE_MU / (den * den);
+        we = w * (-C_X * r43 * F);
+        v0 = w * (-C_X * c * ((4.0 / 3.0) * F - (8.0 / 3.0) * s2 * Fp));
+        const double vs = -C_X * Fp / (4.0 * K_S * r43);
+        v1 = 2.0 * w * vs * dx;
+        v2 = 2.0 * w * vs * dy;
+        v3 = 2.0 * w * vs * dz;
+      }
+    }
+    wv_s[g] = v0;
+    if (GGA) {
+      wv_s[n_pad + g] = v1;
+      wv_s[2 * n_pad + g] = v2;
+      wv_s[3 * n_pad + g] = v3;
+    }
+  }
+  red[threadIdx.x] = we;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {  // fixed tree: bitwise reproducible
+    if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) epart[blockIdx.x] = red[0];
+}
+
+__global__ void __launch_bounds__(1024) k_sum_partials(const double* __restrict__ part, int n, double* __restrict__ out) {
+  __shared__ double red[1024];
+  double a = 0.0;
+  for (int i = threadIdx.x; i < n; i += 1024) a += part[i];
+  red[threadIdx.x] = a;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[0] = red[0];
+}
+
+// ===================================================================================== permutations
+__global__ void k_unpermute_rho(const int32_t* __restrict__ perm, int64_t n_pad, int64_t n_pts,
+                                const double* __restrict__ rho_s, const double* __restrict__ drho_s,
+                                double* __restrict__ rho, double* __restrict__ drho) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pad) return;
+  const int64_t g = perm[i];
+  if (g < 0) return;
+  rho[g] = rho_s[i];
+  if (drho)
+    for (int c = 0; c < 3; ++c) drho[c * n_pts + g] = drho_s[c * n_pad + i];
+}
+
+__global__ void k_gather_wv(const int32_t* __restrict__ perm, int64_t n_pad, int64_t n_pts, int ncomp,
+                            const double* __restrict__ wv, double* __restrict__ wv_s) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pad) return;
+  const int64_t g = perm[i];
+  for (int c = 0; c < ncomp; ++c) wv_s[c * n_pad + i] = (g >= 0) ? wv[c * n_pts + g] : 0.0;
+}
+
+// GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi on the stored tiles (same layout as Phi)
+__global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off,
+                                                 int64_t n_pad, const double* __restrict__ wv_s,
+                                                 const double* __restrict__ phi, const double* __restrict__ d0,
+                                                 const double* __restrict__ d1, const double* __restrict__ d2,
+                                                 double* __restrict__ z) {
+  const int p = blockIdx.x, t = threadIdx.x;
+  const int64_t g = (int64_t)p * GB + t;
+  const double w0 = 0.5 * wv_s[g], w1 = wv_s[n_pad + g], w2 = wv_s[2 * n_pad + g], w3 = wv_s[3 * n_pad + g];
+  const int64_t o0 = panel_off[p] * GB + t;
+  const int K = kp[p];
+  for (int k = 0; k < K; ++k) {
+    const int64_t o = o0 + (int64_t)k * GB;
+    z[o] = w0 * phi[o] + w1 * d0[o] + w2 * d1[o] + w3 * d2[o];
+  }
+}
+
+// ===================================================================================== H4
+namespace vx {
+constexpr int NST = 3;
+constexpr int TW = 64;        // max packed columns per output tile side
+constexpr int KH = 64;        // grid rows (K) per stage: half a grid block
+constexpr int LDH = KH + 4;   // padded leading dimension
+constexpr int OP_BYTES = TW * LDH * 8;  // 34,816
+constexpr int STAGE_BYTES = 2 * OP_BYTES + KH * 8;
+constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
+enum { F_DONE = 1, F_DIAG = 2, F_HALF1 = 4 };
+}  // namespace vx
+
+template <bool GGA>
+__global__ void __launch_bounds__(288, 1)
+    k_vxc(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
+          const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
+          const double* __restrict__ phi, const double* __restrict__ zmat, const double* __restrict__ wv_s, int n_ao,
+          double* __restrict__ Vp) {
+  using namespace vx;
+  extern __shared__ __align__(128) unsigned char smem[];
+  int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
+  const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      mbar_init(bar0 + 8 * (NST + s), 8);
+    }
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  if (warp == 8) {
+    // ------------------------------------------------------------------ producer warp
+    int s = 0;
+    uint32_t ph = 0;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(ticket, 1);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t >= n_tasks) break;
+      const int p = tasks[t];
+      const int K8 = (kp[p] + 7) & ~7;
+      const int64_t base = panel_off[p];
+      const int nt = (K8 + TW - 1) / TW;
+      const int W = (((K8 + nt - 1) / nt) + 7) & ~7;
+      for (int i = 0; i < nt; ++i) {
+        const int i0 = i * W, wi = min(W, K8 - i0);
+        for (int j = GGA ? 0 : i; j < nt; ++j) {
+          const int j0 = j * W, wj = min(W, K8 - j0);
+          const bool diag = !GGA && (i == j);
+          for (int h = 0; h < 2; ++h) {
+            mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+            const uint32_t full = bar0 + 8 * s;
+            if (lane == 0) {
+              hdr[4 * s + 0] = p;
+              hdr[4 * s + 1] = i0 | (j0 << 16);
+              hdr[4 * s + 2] = (wi >> 3) | ((wj >> 3) << 8) | (((diag ? F_DIAG : 0) | (h ? F_HALF1 : 0)) << 16);
+              mbar_arrive_expect_tx(full, (uint32_t)((wi + (diag ? 0 : wj)) * (KH * 8) + (GGA ? 0 : KH * 8)));
+            }
+            __syncwarp();
+            const uint32_t sa = smem_u32(smem + s * STAGE_BYTES), sb = sa + OP_BYTES, sw = sb + OP_BYTES;
+            for (int c = lane; c < wi; c += 32)
+              bulk_g2s(sa + c * (LDH * 8), phi + (base + i0 + c) * GB + h * KH, KH * 8, full);
+            if (!diag) {
+              const double* src = GGA ? zmat : phi;
+              for (int c = lane; c < wj; c += 32)
+                bulk_g2s(sb + c * (LDH * 8), src + (base + j0 + c) * GB + h * KH, KH * 8, full);
+            }
+            if (!GGA && lane == 0) bulk_g2s(sw, wv_s + (int64_t)p * GB + h * KH, KH * 8, full);
+            if (++s == NST) { s = 0; ph ^= 1; }
+          }
+        }
+      }
+    }
+    mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+    if (lane == 0) {
+      hdr[4 * s + 2] = F_DONE << 16;
+      mbar_arrive(bar0 + 8 * s);
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumer warps: 16 x 32 sub-tiles
+  const int wm = warp & 3, wn = warp >> 2, q4 = lane >> 2, r4 = lane & 3;
+  double acc[2][4][2];
+  int s = 0;
+  uint32_t ph = 0;
+  for (;;) {
+    mbar_wait(bar0 + 8 * s, ph);
+    const int p = hdr[4 * s + 0], ij = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
+    const int fl = h2 >> 16;
+    if (fl & F_DONE) break;
+    const int wi = (h2 & 0xff) << 3, wj = ((h2 >> 8) & 0xff) << 3;
+    if (!(fl & F_HALF1)) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
+    }
+    const int m0 = 16 * wm, nb = 32 * wn;
+    const int nj = min(4, max(0, (wj - nb) >> 3));  // active 8-column sub-tiles of this warp
+    if (m0 < wi && nj > 0) {
+      const bool m1 = (m0 + 8 < wi);
+      const double* As = reinterpret_cast<const double*>(smem + s * STAGE_BYTES);
+      const double* Bs = (fl & F_DIAG) ? As : reinterpret_cast<const double*>(smem + s * STAGE_BYTES + OP_BYTES);
+      const double* ws = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + 2 * OP_BYTES) + r4;
+      const double* pa = As + (m0 + q4) * LDH + r4;
+      const double* pb = Bs + (nb + q4) * LDH + r4;
+#pragma unroll 4
+      for (int ks = 0; ks < KH / 4; ++ks) {
+        double a0 = pa[4 * ks], a1 = m1 ? pa[8 * LDH + 4 * ks] : 0.0;
+        if (!GGA) {
+          const double w = ws[4 * ks];
+          a0 *= w;
+          a1 *= w;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (j < nj) {
+            const double b = pb[j * 8 * LDH + 4 * ks];
+            dmma884(acc[0][j][0], acc[0][j][1], a0, b);
+            if (m1) dmma884(acc[1][j][0], acc[1][j][1], a1, b);
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    if (++s == NST) { s = 0; ph ^= 1; }
+
+    if (fl & F_HALF1) {
+      // scatter-accumulate the packed tile into the plan-order matrix (upper triangle for LDA)
+      const int K = kp[p];
+      const int64_t base = panel_off[p];
+      const int i0 = ij & 0xffff, j0 = ij >> 16;
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) {
+        const int r = i0 + m0 + 8 * mi + q4;
+        if (m0 + 8 * mi < wi && r < K) {
+          const int64_t ci = (int64_t)colidx[base + r] * n_ao;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            if (j < nj) {
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const int c = j0 + nb + 8 * j + 2 * r4 + e;
+                if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + colidx[base + c], acc[mi][j][e]);
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+// ===================================================================================== H5
+template <bool GGA>
+__global__ void k_finalise_V(const double* __restrict__ Vp, const int32_t* __restrict__ ao_perm, int n,
+                             double* __restrict__ V) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= n) return;
+  double v;
+  if (GGA)
+    v = Vp[(int64_t)i * n + j] + Vp[(int64_t)j * n + i];  // V = B + B^T (commutative: exactly symmetric)
+  else
+    v = (i <= j) ? Vp[(int64_t)i * n + j] : Vp[(int64_t)j * n + i];
+  V[(int64_t)ao_perm[i] * n + ao_perm[j]] = v;
+}
+
+// ===================================================================================== launchers
+static int g_attr_done = 0;
+static kldi_status set_attrs() {
+  if (g_attr_done) return KLDI_OK;
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_vxc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_vxc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
+  g_attr_done = 1;
+  return KLDI_OK;
+}
+
+kldi_status launch_permute_D(kldi_plan* P, const double* D) {
+  dim3 grid((P->n_ao + 255) / 256, P->n_ao);
+  k_permute_D<<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_rho(kldi_plan* P, bool gga) {
+  kldi_status rc = set_attrs();
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
+  if (gga) KLDI_CUDA(cudaMemsetAsync(P->d_drho_s, 0, sizeof(double) * 3 * P->n_pad, P->stream));
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  if (gga)
+    k_rho<true><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
+                                                           P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
+                                                           P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
+                                                           P->n_pad);
+  else
+    k_rho<false><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
+                                                            P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
+                                                            nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho) {
+  const int nb = (int)((P->n_pad + 255) / 256);
+  k_unpermute_rho<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, P->d_rho_s, P->d_drho_s, rho, drho);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_xc(kldi_plan* P, kldi_functional f) {
+  const int nb = (int)((P->n_pad + 255) / 256);
+  if (f == KLDI_GGA_PBEX)
+    k_xc<true><<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_rho_s, P->d_drho_s, P->d_gw, P->d_wv_s, P->d_epart);
+  else
+    k_xc<false><<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_rho_s, nullptr, P->d_gw, P->d_wv_s, P->d_epart);
+  KLDI_CUDA(cudaGetLastError());
+  k_sum_partials<<<1, 1024, 0, P->stream>>>(P->d_epart, nb, P->d_E);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga) {
+  const int nb = (int)((P->n_pad + 255) / 256);
+  k_gather_wv<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, gga ? 4 : 1, wv, P->d_wv_s);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_vxc(kldi_plan* P, bool gga) {
+  kldi_status rc = set_attrs();
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  if (gga) {
+    k_build_z<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_kp, P->d_panel_off, P->n_pad, P->d_wv_s, P->d_phi,
+                                                       P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_z);
+    KLDI_CUDA(cudaGetLastError());
+    k_vxc<true><<<grid, 288, vx::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
+                                                          P->d_colidx, P->d_phi, P->d_z, P->d_wv_s, P->n_ao, P->d_Vp);
+  } else {
+    k_vxc<false><<<grid, 288, vx::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
+                                                           P->d_panel_off, P->d_colidx, P->d_phi, nullptr, P->d_wv_s,
+                                                           P->n_ao, P->d_Vp);
+  }
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V) {
+  dim3 grid((P->n_ao + 255) / 256, P->n_ao);
+  if (gga)
+    k_finalise_V<true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V);
+  else
+    k_finalise_V<false><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+}  // namespace kldi

@@ -1,0 +1,103 @@
+// Internal declarations of libkldi (not part of the ABI).  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "kldi.h"
+
+namespace kldi {
+
+constexpr int GB = 128;  // points per grid block (BASELINE.json; PAPER.md:118 uses d = 32)
+
+void set_error(const char* fmt, ...);
+
+#define KLDI_CUDA(call)                                                                     \
+  do {                                                                                      \
+    cudaError_t e__ = (call);                                                               \
+    if (e__ != cudaSuccess) {                                                               \
+      kldi::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+      return e__ == cudaErrorMemoryAllocation ? KLDI_ENOMEM : KLDI_ECUDA;                   \
+    }                                                                                       \
+  } while (0)
+
+// Device-side view of the basis in the plan's spatial shell order.
+struct ShellTable {
+  const double* atom_xyz;    // [n_atoms][3]
+  const int32_t* sh_atom;    // [n_shells]
+  const int32_t* sh_l;       // [n_shells]
+  const int32_t* sh_prim0;   // [n_shells+1]
+  const int32_t* sh_ao0;     // [n_shells+1] first plan-order AO of the shell
+  const double* prim_alpha;  // [n_prim]
+  const double* prim_cn;     // [n_prim] coef * (2a/pi)^{3/4} (4a)^{l/2}
+};
+
+}  // namespace kldi
+
+struct kldi_plan {
+  cudaStream_t stream = nullptr;
+  int device = 0, n_sm = 0;
+  double eps = 0.0;
+  int want_grad = 0;
+  int32_t n_atoms = 0, n_shells = 0, n_ao = 0, n_prim = 0;
+  int64_t n_pts = 0, n_blocks = 0, n_pad = 0;
+  kldi_stats stats{};
+
+  // ---- basis (device), plan order
+  double* d_atom_xyz = nullptr;
+  int32_t *d_sh_atom = nullptr, *d_sh_l = nullptr, *d_sh_prim0 = nullptr, *d_sh_ao0 = nullptr;
+  double *d_prim_alpha = nullptr, *d_prim_cn = nullptr;
+  int32_t *d_shell_perm = nullptr, *d_ao_perm = nullptr;  // plan index -> caller index
+  int32_t* d_ao_atom = nullptr;                           // plan AO -> plan atom rank
+
+  // ---- grid (device), Morton order, SoA, padded to n_pad = n_blocks*128
+  double *d_gx = nullptr, *d_gy = nullptr, *d_gz = nullptr, *d_gw = nullptr;
+  int32_t* d_perm_g = nullptr;  // sorted -> caller, -1 = padding
+  uint64_t* d_keys = nullptr;
+
+  // ---- BCS(R) / BCS(C)
+  int32_t *d_row_ptr = nullptr, *d_col_idx = nullptr, *d_blk_col0 = nullptr;
+  int32_t *d_col_ptr = nullptr, *d_row_idx = nullptr, *d_pos = nullptr;
+  double* d_blk_amax = nullptr;
+  int64_t* d_panel_off = nullptr;  // [n_blocks+1] packed-column offsets (each K_p padded to 8)
+  int32_t *d_kp = nullptr;         // [n_blocks] K_p (unpadded)
+  int32_t* d_colidx = nullptr;     // [total_cols] plan AO index of every packed column (pad -> 0)
+  int64_t total_cols = 0;
+  double* d_phi = nullptr;         // [total_cols + slack][128] column-major tiles
+  double* d_dphi[3] = {nullptr, nullptr, nullptr};
+  double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, same layout as d_phi
+
+  // ---- task lists
+  int32_t* d_tasks = nullptr;  // non-empty grid blocks in Morton order
+  int32_t n_tasks = 0;
+  int32_t* d_ticket = nullptr;  // [4] atomic work counters
+
+  // ---- per-call buffers
+  double *d_Dp = nullptr, *d_Vp = nullptr;  // plan-order D and V accumulators [n_ao][n_ao]
+  double *d_rho_s = nullptr, *d_drho_s = nullptr, *d_wv_s = nullptr;  // sorted order, [n_pad], [3][n_pad], [4][n_pad]
+  double *d_epart = nullptr, *d_E = nullptr;
+  double* d_stage_host = nullptr;  // device staging for kldi_exc_host: D and V
+  double* h_E = nullptr;           // pinned
+  cudaEvent_t ev[8] = {};
+  bool have_timings = false;
+
+  // ---- host copies kept for export / tests
+  std::vector<int32_t> h_row_ptr, h_col_idx, h_blk_col0, h_col_ptr, h_row_idx, h_pos, h_shell_perm, h_ao_perm;
+  std::vector<int64_t> h_panel_off;
+};
+
+namespace kldi {
+// plan.cu
+kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid);
+void plan_free(kldi_plan* P);
+// contract.cu
+kldi_status launch_permute_D(kldi_plan* P, const double* D);
+kldi_status launch_rho(kldi_plan* P, bool gga);
+kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
+kldi_status launch_xc(kldi_plan* P, kldi_functional f);
+kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga);
+kldi_status launch_vxc(kldi_plan* P, bool gga);
+kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V);
+}  // namespace kldi
