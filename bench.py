@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py — EXC evaluations/s of the block-filtered hot path on BASELINE.json configs[3]
+(256 waters, 6,400 AOs, 4,224,000 grid points, LDA Slater, eps = 1e-12), one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--eps 1e-12]
+  python bench.py --impl reference        # the CPU oracle, timed on the host cores (bounded sample)
+
+A "step" is one whole kldi_exc call: D permute -> rho contraction -> functional + energy ->
+V contraction -> V finalise, plan creation excluded (once per geometry,
+PAPER.md:174) and reported beside it.  N > 1 (torchrun): the quadrature grid is sharded over the
+ranks and V, E are all-reduced over NCCL; value = evaluations/s of the whole job.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "exc_evals_per_s"
+UNIT = "evals/s"
+N_SM, FMA_PER_CLK_SM = 148, 64          # B200: FP64 FMA lanes per SM per clock (DMMA.8x8x4 = 256 FMA / 4 clk)
+
+
+def basis_of(wl):
+    return (wl.atom_xyz, wl.shell_atom, wl.shell_l, wl.shell_prim_off, wl.prim_alpha, wl.prim_coef)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "_source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def cpu_oracle_sample(wl, n_sample: int):
+    """The oracle as it stands on a bounded, strided sample of the workload's grid points."""
+    import torch
+
+    from oracle import exc_oracle as O
+
+    idx = np.arange(0, wl.n_pts, max(1, wl.n_pts // n_sample))[:n_sample]
+    t0 = time.perf_counter()
+    O.exc(basis_of(wl), wl.grid_xyz[idx], wl.grid_w[idx], wl.D, wl.functional)
+    dt = time.perf_counter() - t0
+    evals_per_s = (len(idx) / wl.n_pts) / dt
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        cores = os.cpu_count()
+    return {"value": evals_per_s, "unit": UNIT, "cores": min(cores, torch.get_num_threads()) if cores else None,
+            "kind": "oracle",
+            "sample": f"every {max(1, wl.n_pts // n_sample)}-th grid point ({len(idx)} of {wl.n_pts}), dense, "
+                      f"{dt:.1f} s, extrapolated linearly in n_pts"}, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2605_10363_b200 import workloads as W
+
+    wl = W.named_config(args.config, eps=args.eps, becke_backend="auto")
+    n_sample = args.ref_sample
+    times = []
+    base = None
+    for i in range(args.warmup + args.steps):
+        base, dt = cpu_oracle_sample(wl, n_sample)
+        if i >= args.warmup:
+            times.append(dt)
+    dt = float(np.mean(times))
+    val = (min(n_sample, wl.n_pts) / wl.n_pts) / dt
+    base["value"] = val
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / val, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args, wl)}, "cpu_baseline": base,
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def workload_name(args, wl):
+    return (f"{args.config}: {wl.name}, {wl.n_atoms} atoms, {wl.n_ao} AOs, {wl.n_pts} grid points, "
+            f"{wl.functional.upper()}, eps={args.eps:g}, D=2QQ^T")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="kldi", choices=["kldi", "reference"])
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--eps", type=float, default=1e-12)
+    ap.add_argument("--ref-sample", type=int, default=4096)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "kldi" else args.warmup
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import __graft_entry__ as G
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the kldi path has no CPU fallback (use --impl reference)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if local == 0:
+        G.build()
+    if world > 1:
+        dist.barrier()
+
+    from paper_2605_10363_b200 import binding as K
+    from paper_2605_10363_b200 import sharding
+    from paper_2605_10363_b200 import workloads as W
+
+    t0 = time.perf_counter()
+    wl_full = W.named_config(args.config, eps=args.eps)
+    gen_s = time.perf_counter() - t0
+    wl = wl_full
+    if world > 1:
+        wl, _ = sharding.shard_workload(wl_full, rank, world)
+    gga = wl.functional == "gga"
+    func = K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER
+    plan = K.Plan.from_workload(wl)
+    st = plan.stats.as_dict()
+    D = torch.as_tensor(wl.D, device="cuda")
+    V = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")
+
+    def step():
+        E, _ = plan.exc(D, func, out=V)
+        if world > 1:
+            E, _ = sharding.allreduce_exc(E, V)
+        return E
+
+    for _ in range(args.warmup):
+        E = step()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage_ms = {}
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(torch.cuda.current_device()) as cs:
+        ev0.record()
+        for _ in range(args.steps):
+            E = step()
+            for k, v in plan.last_timings().items():
+                stage_ms[k] = stage_ms.get(k, 0.0) + v / args.steps
+        ev1.record()
+        torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = 1e3 / ms_per_step
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of D and D2H of V inside the timed region
+    e2e = None
+    if world == 1:
+        Dh = torch.as_tensor(wl.D).pin_memory()
+        Vh = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64).pin_memory()
+        for _ in range(2):
+            plan.exc_host(Dh, func, Vh)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            plan.exc_host(Dh, func, Vh)
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / args.steps
+        nn = wl.n_ao * wl.n_ao * 8
+        e2e = {"value": 1.0 / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nn, "d2h_bytes_per_step": nn + 8,
+               "ms_per_step": e2e_s * 1e3}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    fp64_clock_peak = N_SM * FMA_PER_CLK_SM * 2 * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    try:
+        dmma_live = K.fp64_peak("dmma", 20000)
+    except Exception:
+        dmma_live = None
+    f_rho, f_v = st["flops_rho_useful"], st["flops_v_useful"]
+    f_total = f_rho + f_v
+    t_rho = stage_ms["rho"] * 1e-3
+    roof = {"bound": "tensor", "kernel": "k_rho (rho contraction, DMMA.8x8x4)",
+            "achieved": f_rho / t_rho / 1e12, "peak": fp64_clock_peak, "unit": "TFLOP/s",
+            "frac": f_rho / t_rho / 1e12 / fp64_clock_peak,
+            "peak_source": "FP64 tensor peak derived from unit counts: 148 SMs x 64 FMA/clk x 2 x sm_max_mhz of "
+                           f"MEASURED_PEAKS.json ({pk['_source']}); live DMMA microbenchmark "
+                           f"{dmma_live and round(dmma_live, 2)} TFLOP/s; bf16-ratio rule would give "
+                           f"{pk['bf16_tflops'] * 40.0 / 2250.0:.1f}",
+            "flops_per_launch": f_rho, "exec_flops_per_launch": st["flops_rho_exec"],
+            "launch_ms": stage_ms["rho"], "traffic": None,
+            "v_kernel": {"achieved": f_v / (stage_ms["vxc"] * 1e-3) / 1e12, "launch_ms": stage_ms["vxc"],
+                         "flops_per_launch": f_v, "exec_flops_per_launch": st["flops_v_exec"]}}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tr):
+        try:
+            with open(tr) as f:
+                roof["traffic"] = json.load(f).get(args.config, {}).get("k_rho_dram_bytes")
+        except Exception:
+            pass
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args, wl_full), "l2": "inputs_larger_than_l2 (Phi store "
+                   f"{st['phi_bytes'] / 1e9:.1f} GB, D {wl.n_ao ** 2 * 8 / 1e6:.0f} MB)",
+                   "parallelism": "single GPU" if world == 1 else f"grid sharded over {world} ranks + NCCL all-reduce of V,E"},
+        "grid_points_per_s": wl_full.n_pts * value,
+        "retained_block_tflops": f_total * world / (ms_per_step * 1e-3) / 1e12 if world == 1 else None,
+        "retained_block_frac_of_fp64_peak": f_total / (ms_per_step * 1e-3) / 1e12 / fp64_clock_peak if world == 1 else None,
+        "retained_block_frac_of_nominal_40tf": f_total / (ms_per_step * 1e-3) / 1e12 / 40.0 if world == 1 else None,
+        "flops": {"rho_useful": f_rho, "v_useful": f_v, "rho_exec": st["flops_rho_exec"], "v_exec": st["flops_v_exec"],
+                  "dense_one_product": st["flops_dense"], "retained_over_dense": f_total / (2 * st["flops_dense"]),
+                  "v_symmetry_halving": not gga, "ao_partition": "one AO block per shell"},
+        "stage_ms": stage_ms, "plan_create_s": st["plan_seconds"], "workload_gen_s": gen_s, "exc_energy": E,
+        "plan": {k: st[k] for k in ("n_blocks", "n_blocks_nonempty", "retained_blocks", "candidate_blocks", "sum_k",
+                                     "max_k", "phi_bytes")},
+        "gpu_launches": 6 + (1 if gga else 0), "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -164,6 +164,11 @@ kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, d
  * iterations; returns achieved TFLOP/s (device-timed) in *tflops.  kind 0 = DMMA, 1 = DFMA. */
 kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);
 
+/* Eq. 20 as the plan applies it, on the host, no GPU needed: the 60-bit key
+ * m = sum_k z_k 2^{3k} + y_k 2^{3k+1} + x_k 2^{3k+2} of trunc(128*(xyz - origin)) per axis, each clamped
+ * to [0, 2^20-1].  xyz, origin: HOST [3]. */
+uint64_t kldi_morton_key(const double* xyz, const double* origin);
+
 const char* kldi_last_error(void);
 
 #ifdef __cplusplus

@@ -21,7 +21,7 @@ KLDI_GGA_PBEX = 1
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
-    "kldi_last_error",
+    "kldi_morton_key", "kldi_last_error",
 ]
 
 
@@ -81,8 +81,10 @@ def lib():
         L.kldi_plan_export_tile.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_int64,
                                             C.POINTER(C.c_int32)]
         L.kldi_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.kldi_morton_key.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.kldi_morton_key.restype = C.c_uint64
         for name in EXPORTED:
-            if name != "kldi_last_error":
+            if name not in ("kldi_last_error", "kldi_morton_key"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -227,6 +229,13 @@ class Plan:
         _check(lib().kldi_plan_export_tile(self._h, int(entry), int(comp), C.c_void_p(buf.ctypes.data), buf.nbytes,
                                            C.byref(w)), "kldi_plan_export_tile")
         return buf[: w.value].copy()
+
+
+def morton_key(xyz, origin) -> int:
+    """Host evaluation of Eq. 20 as the plan applies it (no GPU needed)."""
+    a = (C.c_double * 3)(*[float(v) for v in xyz])
+    o = (C.c_double * 3)(*[float(v) for v in origin])
+    return int(lib().kldi_morton_key(a, o))
 
 
 def fp64_peak(kind: str = "dmma", iters: int = 20000) -> float:

@@ -39,6 +39,10 @@ __host__ __device__ inline uint64_t morton_key(double x, double y, double z, dou
   return (spread3(q(x - x0)) << 2) | (spread3(q(y - y0)) << 1) | spread3(q(z - z0));
 }
 
+uint64_t morton_key_host(double x, double y, double z, double x0, double y0, double z0) {
+  return morton_key(x, y, z, x0, y0, z0);
+}
+
 __global__ void k_morton_keys(const double* __restrict__ xyz, int64_t n, int64_t n_pad, double x0, double y0,
                               double z0, uint64_t* __restrict__ keys, int32_t* __restrict__ idx) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

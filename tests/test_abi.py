@@ -1,0 +1,107 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/kldi.h declares,
+fails loudly without a GPU, and its host-side Morton key (Eq. 20) is the
+bit interleave the paper defines."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import __graft_entry__ as g
+
+    g.build()
+    from paper_2605_10363_b200 import binding
+
+    return binding.lib()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    text = open(os.path.join(ROOT, "include", "kldi.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = set(re.findall(r"\b(kldi_[a-z0-9_]+)\s*\(", text))
+    assert {"kldi_plan_create", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc"} <= declared
+    from paper_2605_10363_b200 import binding
+
+    assert declared == set(binding.EXPORTED)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_stats_struct_layout_matches_header():
+    """The ctypes mirror of kldi_stats must have the header's field order and types."""
+    from paper_2605_10363_b200 import binding
+
+    text = open(os.path.join(ROOT, "include", "kldi.h")).read()
+    body = re.search(r"typedef struct \{([^}]*)\} kldi_stats;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = re.findall(r"(int64_t|int32_t|double)\s+([a-z_0-9]+)\s*;", body)
+    cmap = {"int64_t": C.c_int64, "int32_t": C.c_int32, "double": C.c_double}
+    assert [(n, cmap[t]) for t, n in fields] == list(binding.Stats._fields_)
+
+
+def test_no_gpu_means_loud_failure(lib):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2605_10363_b200 import binding, workloads
+
+    wl = workloads.named_config("cfg0")
+    with pytest.raises(binding.KldiError):
+        binding.Plan.from_workload(wl)
+    # and directly at the C boundary: status KLDI_ECUDA (-3) with a message, no plan
+    ax = np.zeros((1, 3)); sa = np.zeros(1, np.int32); sl = np.zeros(1, np.int32); so = np.array([0, 1], np.int32)
+    al = np.ones(1); co = np.ones(1); gx = np.zeros((4, 3)); gw = np.ones(4)
+    atoms = binding._Atoms(1, ax.ctypes.data)
+    shells = binding._Shells(1, sa.ctypes.data, sl.ctypes.data, so.ctypes.data, al.ctypes.data, co.ctypes.data)
+    grid = binding._Grid(4, gx.ctypes.data, gw.ctypes.data)
+    h = C.c_void_p()
+    rc = lib.kldi_plan_create(C.byref(atoms), C.byref(shells), C.byref(grid), 1e-12, 0, None, C.byref(h))
+    assert rc == -3 and not h.value
+    assert b"no CUDA device" in lib.kldi_last_error()
+
+
+def test_invalid_arguments_are_rejected(lib):
+    h = C.c_void_p()
+    assert lib.kldi_plan_create(None, None, None, 1e-12, 0, None, C.byref(h)) == -1
+    assert lib.kldi_plan_stats(None, None) == -1
+    assert lib.kldi_plan_destroy(None) == 0
+    assert lib.kldi_eval_rho(None, None, None, None) == -1
+    assert lib.kldi_build_vxc(None, None, 0, None) == -1
+    e = C.c_double()
+    assert lib.kldi_exc(None, None, 0, C.byref(e), None) == -1
+
+
+def _interleave_bruteforce(ix, iy, iz):
+    m = 0
+    for k in range(20):
+        m |= ((iz >> k) & 1) << (3 * k)
+        m |= ((iy >> k) & 1) << (3 * k + 1)
+        m |= ((ix >> k) & 1) << (3 * k + 2)
+    return m
+
+
+def test_morton_key_is_eq20(lib):
+    from paper_2605_10363_b200 import binding
+
+    rng = np.random.default_rng(7)
+    origin = np.array([-3.0, 2.5, -100.0])
+    pts = origin + rng.uniform(0.0, 8000.0, size=(300, 3)) * rng.uniform(0, 1, size=(300, 1)) ** 3
+    for p in pts:
+        q = [int(np.trunc((p[c] - origin[c]) * 128.0)) for c in range(3)]
+        q = [min(max(v, 0), 2 ** 20 - 1) for v in q]
+        assert binding.morton_key(p, origin) == _interleave_bruteforce(*q)
+    # single-axis unit steps land on the documented bit positions; x is the most significant
+    assert binding.morton_key([1 / 128, 0, 0], [0, 0, 0]) == 4
+    assert binding.morton_key([0, 1 / 128, 0], [0, 0, 0]) == 2
+    assert binding.morton_key([0, 0, 1 / 128], [0, 0, 0]) == 1
+    assert binding.morton_key([1e9, 1e9, 1e9], [0, 0, 0]) == 2 ** 60 - 1      # clamped to 20 bits per axis
+    assert binding.morton_key([-5.0, -5.0, -5.0], [0, 0, 0]) == 0              # below the origin -> 0
+    # locality: points inside one 1/128-bohr cell share a key
+    assert binding.morton_key([0.5001, 0.2501, 0.1251], [0, 0, 0]) == binding.morton_key([0.5003, 0.2503, 0.1253], [0, 0, 0])

@@ -1,0 +1,343 @@
+"""GPU parity: the CUDA path behind the C ABI against the CPU oracle, element by element on the
+same seeded inputs (tolerances of BASELINE.json north_star: max|d rho| <= 1e-9, max|dV| <= 1e-9,
+|dE| <= 1e-8 Ha at eps = 1e-12), plus the structural invariants of the plan (Eq. 20, Eq. 12,
+BCS(R)/BCS(C)) and the edge cases."""
+import numpy as np
+import pytest
+
+from oracle import exc_oracle as O
+from paper_2605_10363_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHO, TOL_V, TOL_E = 1e-9, 1e-9, 1e-8
+
+
+def basis_of(wl):
+    return (wl.atom_xyz, wl.shell_atom, wl.shell_l, wl.shell_prim_off, wl.prim_alpha, wl.prim_coef)
+
+
+@pytest.fixture(scope="module")
+def K():
+    import torch
+
+    assert torch.cuda.is_available()
+    from paper_2605_10363_b200 import binding
+
+    binding.lib()  # raises if libkldi.so is missing: no fallback
+    return binding
+
+
+def run_gpu(K, wl, eps=None):
+    import torch
+
+    gga = wl.functional == "gga"
+    plan = K.Plan.from_workload(wl, eps=eps)
+    D = torch.as_tensor(wl.D, device="cuda")
+    E, V = plan.exc(D, K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER)
+    if gga:
+        rho, drho = plan.eval_rho(D, want_grad=True)
+        drho = drho.cpu().numpy()
+    else:
+        rho, drho = plan.eval_rho(D), None
+    out = {"E": E, "V": V.cpu().numpy(), "rho": rho.cpu().numpy(), "drho": drho, "plan": plan}
+    return out
+
+
+def check(out, ref, tol_scale=1.0):
+    assert np.max(np.abs(out["rho"] - ref["rho"])) <= TOL_RHO * tol_scale
+    assert np.max(np.abs(out["V"] - ref["V"])) <= TOL_V * tol_scale
+    assert abs(out["E"] - ref["E"]) <= TOL_E * tol_scale
+    assert np.array_equal(out["V"], out["V"].T)          # exactly symmetric (reading A15)
+    if ref.get("drho") is not None:
+        assert np.max(np.abs(out["drho"] - ref["drho"])) <= TOL_RHO * tol_scale
+
+
+CASES = [
+    ("cfg0", None, "lda"), ("cfg0", None, "gga"),
+    ("cfg1", 8, "lda"), ("cfg2", 6, "lda"), ("cfg3", 12, "lda"), ("cfg4", 6, "gga"),
+]
+
+
+@pytest.mark.parametrize("name,n,fn", CASES)
+def test_parity_reduced_configs(K, name, n, fn):
+    """Same recipe and seed as BASELINE.json configs[0..4], molecule count reduced so the dense
+    oracle finishes in seconds; spans many grid blocks, a ragged last block and ragged K_p."""
+    wl = W.named_config(name, n_override=n, functional=fn)
+    out = run_gpu(K, wl)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, fn)
+    check(out, ref)
+    st = out["plan"].stats
+    assert st.n_blocks == (wl.n_pts + 127) // 128 and st.n_ao == wl.n_ao
+    assert 0 < st.retained_blocks <= st.candidate_blocks
+    out["plan"].close()
+
+
+def test_parity_cfg1_full(K):
+    """BASELINE.json configs[1] at full size (32 waters, 800 AOs, 528,000 points), element by element."""
+    wl = W.named_config("cfg1")
+    out = run_gpu(K, wl)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda")
+    check(out, ref)
+    st = out["plan"].stats
+    assert st.flops_rho_useful < 0.2 * st.flops_dense      # the filter must actually remove work
+    out["plan"].close()
+
+
+def test_dense_limit_equals_oracle_to_roundoff(K):
+    """eps -> 0: the block-filtered products are the dense products (Eq. 16 -> Eq. 7)."""
+    for fn in ("lda", "gga"):
+        wl = W.named_config("cfg1", n_override=3, functional=fn)
+        out = run_gpu(K, wl, eps=0.0)
+        ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, fn)
+        assert out["plan"].stats.retained_blocks == out["plan"].stats.candidate_blocks
+        assert np.max(np.abs(out["rho"] - ref["rho"])) <= 1e-12
+        assert np.max(np.abs(out["V"] - ref["V"])) <= 1e-12
+        assert abs(out["E"] - ref["E"]) <= 1e-12
+        out["plan"].close()
+
+
+def test_screening_error_grows_with_eps(K):
+    """the error is controlled by the threshold and grows with it."""
+    wl = W.named_config("cfg1", n_override=8)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda")
+    errs, kept = [], []
+    for eps in (1e-14, 1e-10, 1e-6, 1e-3):
+        out = run_gpu(K, wl, eps=eps)
+        errs.append(np.max(np.abs(out["rho"] - ref["rho"])))
+        kept.append(out["plan"].stats.retained_blocks)
+        out["plan"].close()
+    assert kept[0] > kept[1] > kept[2] > kept[3]
+    assert errs[0] <= 1e-11 and errs[1] <= 1e-8
+    assert errs[3] > errs[2] > errs[1]
+
+
+def test_eval_rho_and_build_vxc_separately(K):
+    import torch
+
+    for fn in ("lda", "gga"):
+        wl = W.named_config("cfg4", n_override=4, functional=fn)
+        ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, fn)
+        plan = K.Plan.from_workload(wl)
+        V = plan.build_vxc(torch.as_tensor(ref["wv"], device="cuda"), gga=(fn == "gga"))
+        assert np.max(np.abs(V.cpu().numpy() - ref["V"])) <= TOL_V
+        # a wv of mixed sign, unrelated to any density
+        rng = np.random.default_rng(3)
+        wv = rng.standard_normal(ref["wv"].shape) * wl.grid_w
+        V2 = plan.build_vxc(torch.as_tensor(wv, device="cuda"), gga=(fn == "gga")).cpu().numpy()
+        if fn == "gga":
+            phi, dphi = O.ao_values(*basis_of(wl), wl.grid_xyz, deriv=True)
+            Vr = O.vxc_gga_from_wv(phi, dphi, wv)
+        else:
+            Vr = O.vxc_lda_from_wv(O.ao_values(*basis_of(wl), wl.grid_xyz), wv)
+        assert np.max(np.abs(V2 - Vr)) <= TOL_V
+        plan.close()
+
+
+def test_plan_structure_invariants(K):
+    """Eq. 20 ordering and the lossless BCS(R)/BCS(C) re-layout."""
+    wl = W.named_config("cfg1", n_override=5)
+    plan = K.Plan.from_workload(wl)
+    perm = plan.export("perm_g")
+    keys = plan.export("morton_keys")
+    n_blocks = int(plan.stats.n_blocks)
+    assert perm.shape[0] == n_blocks * 128
+    real = perm[perm >= 0]
+    assert np.array_equal(np.sort(real), np.arange(wl.n_pts))          # a permutation of the caller's points
+    assert np.all(perm[wl.n_pts:] == -1)                               # padding last
+    assert np.all(np.diff(keys.astype(np.float64)) >= 0) and np.all(keys[:wl.n_pts][1:] >= keys[:wl.n_pts][:-1])
+    origin = wl.grid_xyz.min(axis=0)
+    for i in np.random.default_rng(0).integers(0, wl.n_pts, 200):       # keys are Eq. 20 of the sorted points
+        assert int(keys[i]) == K.morton_key(wl.grid_xyz[perm[i]], origin)
+    same = keys[:wl.n_pts][1:] == keys[:wl.n_pts][:-1]                   # stable sort: ties keep caller order
+    assert np.all(perm[:wl.n_pts][1:][same] > perm[:wl.n_pts][:-1][same])
+    row_ptr, col_idx = plan.export("row_ptr"), plan.export("col_idx")
+    col_ptr, row_idx, pos = plan.export("col_ptr"), plan.export("row_idx"), plan.export("pos")
+    assert row_ptr[0] == 0 and row_ptr[-1] == len(col_idx) == plan.stats.retained_blocks
+    assert np.all(np.diff(row_ptr) >= 0) and np.all(np.diff(col_ptr) >= 0) and col_ptr[-1] == len(row_idx)
+    for p in range(n_blocks):
+        c = col_idx[row_ptr[p]:row_ptr[p + 1]]
+        assert np.all(np.diff(c) > 0) and (len(c) == 0 or (c[0] >= 0 and c[-1] < plan.stats.n_shells))
+    rows_of_entry = np.repeat(np.arange(n_blocks), np.diff(row_ptr))
+    for q in range(plan.stats.n_shells):
+        r = row_idx[col_ptr[q]:col_ptr[q + 1]]
+        assert np.all(np.diff(r) > 0)
+        e = pos[col_ptr[q]:col_ptr[q + 1]]
+        assert np.all(col_idx[e] == q) and np.all(rows_of_entry[e] == r)      # same block set, both layouts
+    assert np.array_equal(np.sort(pos), np.arange(len(col_idx)))
+    sp, ap = plan.export("shell_perm"), plan.export("ao_perm")
+    assert np.array_equal(np.sort(sp), np.arange(len(wl.shell_l))) and np.array_equal(np.sort(ap), np.arange(wl.n_ao))
+    plan.close()
+
+
+@pytest.mark.parametrize("fn", ["lda", "gga"])
+def test_tiles_and_filter_against_oracle_ao_values(K, fn):
+    """P3/P4: stored tiles are the oracle's AO values at the sorted points; the retained set is
+    exactly {(p,q): max|Phi_pq| >= eps} (Eq. 12) up to values within rounding of eps."""
+    wl = W.named_config("cfg0", functional=fn)
+    eps = 1e-8
+    plan = K.Plan.from_workload(wl, eps=eps)
+    perm = plan.export("perm_g")
+    row_ptr, col_idx, amax = plan.export("row_ptr"), plan.export("col_idx"), plan.export("block_amax")
+    sp = plan.export("shell_perm")
+    ao0 = np.concatenate([[0], np.cumsum([(l + 1) * (l + 2) // 2 for l in wl.shell_l])])
+    idx = np.where(perm >= 0, perm, perm[wl.n_pts - 1])
+    if fn == "gga":
+        phi, dphi = O.ao_values(*basis_of(wl), wl.grid_xyz[idx], deriv=True)
+    else:
+        phi, dphi = O.ao_values(*basis_of(wl), wl.grid_xyz[idx]), None
+    n_blocks = int(plan.stats.n_blocks)
+    kept = set()
+    for p in range(n_blocks):
+        for e in range(row_ptr[p], row_ptr[p + 1]):
+            kept.add((p, int(col_idx[e])))
+    n_checked = 0
+    for p in range(n_blocks):
+        rows = slice(128 * p, 128 * p + 128)
+        for q in range(len(sp)):
+            s = sp[q]
+            blk = phi[rows, ao0[s]:ao0[s + 1]]
+            a = np.max(np.abs(blk))
+            if dphi is not None:
+                a = max(a, np.max(np.abs(dphi[:, rows, ao0[s]:ao0[s + 1]])))
+            if abs(a - eps) > 1e-6 * eps:
+                assert ((p, q) in kept) == (a >= eps), (p, q, a)
+    for e in np.random.default_rng(1).integers(0, len(col_idx), 60):
+        p = int(np.searchsorted(row_ptr, e, side="right") - 1)
+        s = sp[col_idx[e]]
+        ref = phi[128 * p:128 * p + 128, ao0[s]:ao0[s + 1]].T
+        tile = plan.export_tile(int(e), 0)
+        assert tile.shape == ref.shape and np.max(np.abs(tile - ref)) <= 1e-14
+        a = np.max(np.abs(ref))
+        if dphi is not None:
+            for c in range(3):
+                refc = dphi[c, 128 * p:128 * p + 128, ao0[s]:ao0[s + 1]].T
+                assert np.max(np.abs(plan.export_tile(int(e), 1 + c) - refc)) <= 1e-13
+                a = max(a, np.max(np.abs(refc)))
+        assert abs(amax[e] - a) <= 1e-14 * max(1.0, a)
+        n_checked += 1
+    assert n_checked == 60
+    plan.close()
+
+
+def test_edge_cases(K):
+    import torch
+
+    wl = W.named_config("cfg0")
+    D = torch.as_tensor(wl.D, device="cuda")
+    basis = basis_of(wl)
+    # (a) a grid so far away that every block is filtered out
+    far = wl.grid_xyz[:300] + 500.0
+    plan = K.Plan(*basis, far, wl.grid_w[:300], 1e-12)
+    assert plan.stats.retained_blocks == 0 and plan.stats.n_blocks_nonempty == 0
+    E, V = plan.exc(D)
+    assert E == 0.0 and float(V.abs().max()) == 0.0 and float(plan.eval_rho(D).abs().max()) == 0.0
+    plan.close()
+    # (b) one point, (c) 129 points (one full block + a block of 1), (d) zero weights
+    for n in (1, 129):
+        pts = wl.grid_xyz[2000:2000 + n]
+        w = wl.grid_w[2000:2000 + n].copy()
+        if n == 129:
+            w[::2] = 0.0
+        plan = K.Plan(*basis, pts, w, 1e-12)
+        E, V = plan.exc(D)
+        ref = O.exc(basis, pts, w, wl.D, "lda")
+        assert abs(E - ref["E"]) <= 1e-12 and np.max(np.abs(V.cpu().numpy() - ref["V"])) <= 1e-12
+        assert np.max(np.abs(plan.eval_rho(D).cpu().numpy() - ref["rho"])) <= 1e-11
+        plan.close()
+    # (e) a minimal basis: one s shell on one atom
+    one = (np.zeros((1, 3)), np.array([0], np.int32), np.array([0], np.int32), np.array([0, 1], np.int32),
+           np.array([0.9]), np.array([1.0]))
+    pts, w = W.atomic_grid(1.0)
+    plan = K.Plan(*one, pts, w, 1e-12)
+    E, V = plan.exc(torch.tensor([[2.0]], dtype=torch.float64, device="cuda"))
+    ref = O.exc(one, pts, w, np.array([[2.0]]), "lda")
+    assert abs(E - ref["E"]) <= 1e-13 and abs(float(V[0, 0]) - ref["V"][0, 0]) <= 1e-13
+    plan.close()
+    # (f) contracted shells and a non-trivial coefficient
+    con = (np.array([[0.0, 0.0, 0.0], [0.0, 0.0, 1.4]]), np.array([0, 0, 1], np.int32), np.array([0, 2, 1], np.int32),
+           np.array([0, 3, 4, 6], np.int32), np.array([3.0, 0.8, 0.2, 0.6, 1.1, 0.3]),
+           np.array([0.3, 0.5, 0.4, 1.0, 0.7, 0.6]))
+    pts = np.vstack([pts, pts + np.array([0.0, 0.0, 1.4])])
+    w2 = np.concatenate([w, w]) * 0.5
+    Dm = W.density_matrix(10, 2, 11)
+    plan = K.Plan(*con, pts, w2, 1e-12, want_gradients=True)
+    E, V = plan.exc(torch.as_tensor(Dm, device="cuda"), K.KLDI_GGA_PBEX)
+    ref = O.exc(con, pts, w2, Dm, "gga")
+    assert abs(E - ref["E"]) <= 1e-12 and np.max(np.abs(V.cpu().numpy() - ref["V"])) <= 1e-12
+    plan.close()
+
+
+def test_errors_on_gpu(K):
+    import torch
+
+    wl = W.named_config("cfg0")
+    plan = K.Plan.from_workload(wl)           # LDA plan: no gradients
+    D = torch.as_tensor(wl.D, device="cuda")
+    with pytest.raises(K.KldiError):
+        plan.exc(D, K.KLDI_GGA_PBEX)
+    with pytest.raises(K.KldiError):
+        plan.eval_rho(D, want_grad=True)
+    with pytest.raises(K.KldiError):
+        plan.eval_rho(D.cpu())
+    E, _ = plan.exc(D)                        # the plan stays usable after a failed call
+    assert E < 0.0
+    plan.close()
+
+
+def test_reproducible_rho_and_energy(K):
+    """rho and E_xc use no atomics: bitwise identical between calls.  V is accumulated with FP64
+    atomics: equal to rounding."""
+    import torch
+
+    wl = W.named_config("cfg1", n_override=6)
+    plan = K.Plan.from_workload(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    E1, V1 = plan.exc(D)
+    r1 = plan.eval_rho(D).clone()
+    E2, V2 = plan.exc(D)
+    r2 = plan.eval_rho(D)
+    assert E1 == E2 and torch.equal(r1, r2)
+    assert float((V1 - V2).abs().max()) <= 1e-14 * float(V1.abs().max())
+    plan.close()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_sampled_parity(K, name):
+    """BASELINE.json configs[3] / configs[4] at FULL size, in the launch configuration bench.py times:
+    rho (and grad rho) at sampled grid points and sampled V entries, each from the plain definition."""
+    import torch
+
+    wl = W.named_config(name)
+    gga = wl.functional == "gga"
+    basis = basis_of(wl)
+    plan = K.Plan.from_workload(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    rng = np.random.default_rng(42)
+    # sample near atoms (where rho is large) and anywhere
+    w_sorted = np.argsort(-np.abs(wl.grid_w))
+    sample = np.unique(np.concatenate([rng.integers(0, wl.n_pts, 96), rng.choice(w_sorted[: wl.n_pts // 4], 96)]))
+    if gga:
+        rho, drho = plan.eval_rho(D, want_grad=True)
+        r_ref, g_ref = O.rho_at_points(basis, wl.grid_xyz[sample], wl.D, want_grad=True)
+        assert np.max(np.abs(drho.cpu().numpy()[:, sample] - g_ref)) <= TOL_RHO
+    else:
+        rho = plan.eval_rho(D)
+        r_ref = O.rho_at_points(basis, wl.grid_xyz[sample], wl.D)
+    assert np.max(np.abs(rho.cpu().numpy()[sample] - r_ref)) <= TOL_RHO
+    assert float(r_ref.max()) > 1e-3
+    # V from a seeded synthetic wv (independent of the CUDA path)
+    shape = (4, wl.n_pts) if gga else (wl.n_pts,)
+    wv = rng.standard_normal(shape) * wl.grid_w
+    V = plan.build_vxc(torch.as_tensor(wv, device="cuda"), gga=gga).cpu().numpy()
+    n = wl.n_ao
+    pairs = [(0, 0), (n - 1, n - 1), (3, 17), (17, 3), (n // 2, n // 2 + 7)] + \
+            [(int(a), int(b)) for a, b in rng.integers(0, n, (7, 2))]
+    ref = O.vxc_entries_from_wv(basis, wl.grid_xyz, wv, pairs, gga=gga)
+    got = np.array([V[a, b] for a, b in pairs])
+    assert np.max(np.abs(got - ref)) <= TOL_V
+    assert np.array_equal(V, V.T)
+    # the whole driver runs at this size and returns a finite, negative exchange energy
+    E, Vx = plan.exc(D, K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER)
+    assert np.isfinite(E) and E < 0.0 and bool(torch.isfinite(Vx).all())
+    plan.close()
