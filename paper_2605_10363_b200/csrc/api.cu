@@ -148,7 +148,7 @@ kldi_status kldi_eval_rho(kldi_plan* P, const double* D, double* rho, double* dr
   kldi_status rc;
   P->have_timings = false;
   EV(0);
-  if ((rc = launch_permute_D(P, D)) != KLDI_OK) return rc;
+  if ((rc = launch_permute_D(P, D, drho != nullptr)) != KLDI_OK) return rc;
   EV(1);
   if ((rc = launch_rho(P, drho != nullptr)) != KLDI_OK) return rc;
   EV(2);
@@ -185,7 +185,7 @@ static kldi_status exc_enqueue(kldi_plan* P, const double* D, kldi_functional f,
   kldi_status rc;
   P->have_timings = false;
   EV(0);
-  if ((rc = launch_permute_D(P, D)) != KLDI_OK) return rc;
+  if ((rc = launch_permute_D(P, D, gga)) != KLDI_OK) return rc;
   EV(1);
   if ((rc = launch_rho(P, gga)) != KLDI_OK) return rc;
   EV(2);

@@ -18,10 +18,20 @@ namespace kldi {
 constexpr int LD = GB + 4;  // padded smem leading dimension of a 128-row column: conflict-free 8-B fragments
 
 // ===================================================================================== H1
+// TRI: the strictly lower triangle of D (plan order), the diagonal halved, zeros above.  D is symmetric, so
+// rho = sum_{mu,nu} D_{mu nu} chi_mu chi_nu = 2 sum_{mu >= nu} D'_{mu nu} chi_mu chi_nu: the rho contraction then
+// only visits the block pairs on one side of the diagonal (the symmetry of PAPER.md:220).
+template <bool TRI>
 __global__ void k_permute_D(const double* __restrict__ D, const int32_t* __restrict__ ao_perm, int n,
                             double* __restrict__ Dp) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
-  if (j < n) Dp[(int64_t)i * n + j] = D[(int64_t)ao_perm[i] * n + ao_perm[j]];
+  if (j >= n) return;
+  double v = 0.0;
+  if (!TRI || j <= i) {
+    v = D[(int64_t)ao_perm[i] * n + ao_perm[j]];
+    if (TRI && j == i) v *= 0.5;
+  }
+  Dp[(int64_t)i * n + j] = v;
 }
 
 // ===================================================================================== H2
@@ -36,23 +46,37 @@ constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
 enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
 }  // namespace rho
 
-template <bool FULL>
+// One ring stage of a consumer warp: nks k-steps of 4, NJ active 8-column groups (compile-time, so that no MMA
+// is predicated: a predicated mma.sync costs a WARPSYNC + NOP pair around every DMMA).
+template <int NJ>
 __device__ __forceinline__ void rho_ksteps(double (&acc)[2][16][2], const double* __restrict__ ps,
-                                           const double* __restrict__ ds, int nks, int nW) {
+                                           const double* __restrict__ ds, int nks) {
+#pragma unroll 2
   for (int ks = 0; ks < nks; ++ks) {
     const double a0 = ps[ks * 4 * LD], a1 = ps[ks * 4 * LD + 8];
+    double b[NJ];
 #pragma unroll
-    for (int j = 0; j < 16; ++j) {
-      if (FULL || j < nW) {
-        const double b = ds[ks * 4 * (rho::NT + 4) + 8 * j];
-        dmma884(acc[0][j][0], acc[0][j][1], a0, b);
-        dmma884(acc[1][j][0], acc[1][j][1], a1, b);
-      }
+    for (int j = 0; j < NJ; ++j) b[j] = ds[ks * 4 * (rho::NT + 4) + 8 * j];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      dmma884(acc[0][j][0], acc[0][j][1], a0, b[j]);
+      dmma884(acc[1][j][0], acc[1][j][1], a1, b[j]);
     }
   }
 }
 
-template <bool GGA>
+__device__ __forceinline__ void rho_stage(double (&acc)[2][16][2], const double* __restrict__ ps,
+                                          const double* __restrict__ ds, int nks, int nj) {
+  switch (nj) {
+#define KLDI_CASE(N) case N: rho_ksteps<N>(acc, ps, ds, nks); break;
+    KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7) KLDI_CASE(8)
+    KLDI_CASE(9) KLDI_CASE(10) KLDI_CASE(11) KLDI_CASE(12) KLDI_CASE(13) KLDI_CASE(14) KLDI_CASE(15) KLDI_CASE(16)
+#undef KLDI_CASE
+    default: break;
+  }
+}
+
+template <bool GGA, bool TRI>
 __global__ void __launch_bounds__(288, 1)
     k_rho(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
@@ -92,21 +116,26 @@ __global__ void __launch_bounds__(288, 1)
         int cn[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) cn[c] = (lane + 32 * c < Wj) ? colidx[base + n0 + lane + 32 * c] : -1;
-        for (int k0 = 0; k0 < K8; k0 += KC) {
+        // TRI: D' is lower triangular in packed order (colidx ascends), so chunk rows k < n0 contribute
+        // nothing to this N-tile and a chunk [k0, k0+kc) only reaches the columns n < k0 + kc.
+        const int kstart = TRI ? (n0 / KC) * KC : 0;
+        for (int k0 = kstart; k0 < K8; k0 += KC) {
           const int kc = min(KC, K8 - k0);
+          const int wact = TRI ? min(Wj, k0 + kc - n0) : Wj;
           mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
           const int rowidx = (lane < kc) ? colidx[base + k0 + lane] : 0;
           const uint32_t full = bar0 + 8 * s;
           if (lane == 0) {
             int fl = 0;
-            if (k0 == 0) fl |= F_FIRST;
+            if (k0 == kstart) fl |= F_FIRST;
             if (k0 + KC >= K8) {
               fl |= F_LAST_TILE;
               if (jt == ntile - 1) fl |= F_LAST_PANEL;
             }
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = n0;
-            hdr[4 * s + 2] = (kc >> 2) | ((Wj >> 3) << 8) | (fl << 16);
+            hdr[4 * s + 2] = (kc >> 2) | ((wact >> 3) << 8) | (fl << 16);
+            hdr[4 * s + 3] = Wj >> 3;
             mbar_arrive_expect_tx(full, (uint32_t)kc * (GB * 8));
           }
           __syncwarp();
@@ -119,7 +148,7 @@ __global__ void __launch_bounds__(288, 1)
             const uint32_t dst = sd + (r * (NT + 4) + lane) * 8;
 #pragma unroll
             for (int c = 0; c < 4; ++c)
-              if (cn[c] >= 0) cp_async8(dst + c * 256, drow + cn[c]);
+              if (cn[c] >= 0 && lane + 32 * c < wact) cp_async8(dst + c * 256, drow + cn[c]);
           }
           cp_async_mbar_arrive_noinc(full);
           if (++s == NST) { s = 0; ph ^= 1; }
@@ -148,17 +177,14 @@ __global__ void __launch_bounds__(288, 1)
     const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
     const int fl = h2 >> 16;
     if (fl & F_DONE) break;
-    const int nks = h2 & 0xff, nW = (h2 >> 8) & 0xff;
+    const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, nW = hdr[4 * s + 3];
     if (fl & F_FIRST) {
 #pragma unroll
       for (int j = 0; j < 16; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
     }
     const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 16 * warp + q4;
     const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
-    if (nW == 16)
-      rho_ksteps<true>(acc, ps, ds, nks, nW);
-    else
-      rho_ksteps<false>(acc, ps, ds, nks, nW);
+    rho_stage(acc, ps, ds, nks, nj);
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
     if (++s == NST) { s = 0; ph ^= 1; }
@@ -193,7 +219,7 @@ __global__ void __launch_bounds__(288, 1)
             if (r4 == 0) {
               const int64_t g = (int64_t)p * GB + 16 * warp + 8 * mi + q4;
               if (c == 0)
-                rho_s[g] = v;
+                rho_s[g] = TRI ? 2.0 * v : v;
               else
                 drho_s[(int64_t)(c - 1) * n_pad + g] = 2.0 * v;
             }
@@ -480,17 +506,20 @@ __global__ void k_finalise_V(const double* __restrict__ Vp, const int32_t* __res
 static int g_attr_done = 0;
 static kldi_status set_attrs() {
   if (g_attr_done) return KLDI_OK;
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_vxc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_vxc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
   g_attr_done = 1;
   return KLDI_OK;
 }
 
-kldi_status launch_permute_D(kldi_plan* P, const double* D) {
+kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
   dim3 grid((P->n_ao + 255) / 256, P->n_ao);
-  k_permute_D<<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
+  if (gga)  // the GGA epilogue needs the full X = Phi D for grad rho; LDA uses the triangular form
+    k_permute_D<false><<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
+  else
+    k_permute_D<true><<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }
@@ -504,12 +533,12 @@ kldi_status launch_rho(kldi_plan* P, bool gga) {
   if (P->n_tasks == 0) return KLDI_OK;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   if (gga)
-    k_rho<true><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
+    k_rho<true, false><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
                                                            P->n_pad);
   else
-    k_rho<false><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
+    k_rho<false, true><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
                                                             nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad);
   KLDI_CUDA(cudaGetLastError());

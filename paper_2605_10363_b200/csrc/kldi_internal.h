@@ -94,7 +94,7 @@ uint64_t morton_key_host(double x, double y, double z, double x0, double y0, dou
 kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid);
 void plan_free(kldi_plan* P);
 // contract.cu
-kldi_status launch_permute_D(kldi_plan* P, const double* D);
+kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
 kldi_status launch_rho(kldi_plan* P, bool gga);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);
