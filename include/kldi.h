@@ -89,13 +89,16 @@ typedef struct {
   int64_t max_k;            /* max_p K_p */
   int64_t phi_bytes;        /* device bytes of the stored Phi (and gradient) tiles */
   int64_t workspace_bytes;  /* other device bytes owned by the plan */
-  double flops_rho_useful;  /* sum_p 2*128*K_p^2            (retained-block FLOPs of one rho build) */
-  double flops_rho_exec;    /* FLOPs the rho kernel issues (padding and symmetry accounted) */
+  double flops_rho_useful;  /* sum_p 2*128*K_p^2: retained-block FLOPs of one rho build without symmetry (GGA form) */
+  double flops_rho_exec;    /* FLOPs the GGA-form rho kernel issues (K_p padded to 8) */
   double flops_v_useful;    /* LDA: sum_p 128*K_p*(K_p+1) (q<=r only); GGA: sum_p 2*128*K_p^2 */
-  double flops_v_exec;      /* FLOPs the V kernel issues (whole tiles, padded) */
+  double flops_v_exec;      /* FLOPs the V kernel issues (16 x 8 MMA units of the schedule, padded) */
   double flops_dense;       /* 2*n_pts*n_ao^2 : one dense product */
   double plan_seconds;      /* wall time of kldi_plan_create */
   double eps;
+  double flops_rho_useful_sym; /* sum_p 128*K_p*(K_p+1): the LDA rho build, which uses D = D^T */
+  double flops_rho_exec_sym;   /* FLOPs the LDA-form (triangular D) rho kernel issues */
+  double flops_v_crit;         /* V kernel: 8 warps x the busiest warp's units, summed (schedule imbalance) */
 } kldi_stats;
 
 /* Once per geometry: Morton reorder of the grid into blocks of 128 (Eq. 20), spatial

@@ -50,6 +50,7 @@ class Stats(C.Structure):
         ("sum_k_pad", C.c_int64), ("max_k", C.c_int64), ("phi_bytes", C.c_int64), ("workspace_bytes", C.c_int64),
         ("flops_rho_useful", C.c_double), ("flops_rho_exec", C.c_double), ("flops_v_useful", C.c_double),
         ("flops_v_exec", C.c_double), ("flops_dense", C.c_double), ("plan_seconds", C.c_double), ("eps", C.c_double),
+        ("flops_rho_useful_sym", C.c_double), ("flops_rho_exec_sym", C.c_double), ("flops_v_crit", C.c_double),
     ]
 
     def as_dict(self) -> dict:

@@ -99,21 +99,23 @@ kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells,
     delete P;
     return KLDI_EINVAL;
   }
-  // FLOPs the kernels issue (whole DMMA tiles)
-  double fr = 0, fv = 0;
+  // FLOPs the rho kernel issues: full form, and the triangular-D form (mirrors the producer loop of k_rho)
+  double fr = 0, frs = 0;
   for (int64_t p = 0; p < P->n_blocks; ++p) {
-    const double k8 = (double)(P->h_panel_off[p + 1] - P->h_panel_off[p]);
-    fr += 2.0 * GB * k8 * k8;
-    const int nt = ((int)k8 + 63) / 64;
-    if (nt) {
-      const int W = ((((int)k8 + nt - 1) / nt) + 7) & ~7;
-      for (int i = 0; i < nt; ++i)
-        for (int j = P->want_grad ? 0 : i; j < nt; ++j)
-          fv += 2.0 * GB * std::min(W, (int)k8 - i * W) * (double)std::min(W, (int)k8 - j * W);
+    const int k8 = (int)(P->h_panel_off[p + 1] - P->h_panel_off[p]);
+    fr += 2.0 * GB * (double)k8 * k8;
+    if (!k8) continue;
+    const int ntile = (k8 + 127) / 128, W = (((k8 + ntile - 1) / ntile) + 7) & ~7;
+    for (int jt = 0; jt < ntile; ++jt) {
+      const int n0 = jt * W, Wj = std::min(W, k8 - n0);
+      for (int k0 = (n0 / 32) * 32; k0 < k8; k0 += 32) {
+        const int kc = std::min(32, k8 - k0);
+        frs += 2.0 * GB * kc * (double)std::min(Wj, k0 + kc - n0);
+      }
     }
   }
   P->stats.flops_rho_exec = fr;
-  P->stats.flops_v_exec = fv;
+  P->stats.flops_rho_exec_sym = frs;
   *out = P;
   return KLDI_OK;
 }

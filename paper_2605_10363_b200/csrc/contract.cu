@@ -316,177 +316,7 @@ __global__ void k_gather_wv(const int32_t* __restrict__ perm, int64_t n_pad, int
   for (int c = 0; c < ncomp; ++c) wv_s[c * n_pad + i] = (g >= 0) ? wv[c * n_pts + g] : 0.0;
 }
 
-// GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi on the stored tiles (same layout as Phi)
-__global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off,
-                                                 int64_t n_pad, const double* __restrict__ wv_s,
-                                                 const double* __restrict__ phi, const double* __restrict__ d0,
-                                                 const double* __restrict__ d1, const double* __restrict__ d2,
-                                                 double* __restrict__ z) {
-  const int p = blockIdx.x, t = threadIdx.x;
-  const int64_t g = (int64_t)p * GB + t;
-  const double w0 = 0.5 * wv_s[g], w1 = wv_s[n_pad + g], w2 = wv_s[2 * n_pad + g], w3 = wv_s[3 * n_pad + g];
-  const int64_t o0 = panel_off[p] * GB + t;
-  const int K = kp[p];
-  for (int k = 0; k < K; ++k) {
-    const int64_t o = o0 + (int64_t)k * GB;
-    z[o] = w0 * phi[o] + w1 * d0[o] + w2 * d1[o] + w3 * d2[o];
-  }
-}
-
-// ===================================================================================== H4
-namespace vx {
-constexpr int NST = 3;
-constexpr int TW = 64;        // max packed columns per output tile side
-constexpr int KH = 64;        // grid rows (K) per stage: half a grid block
-constexpr int LDH = KH + 4;   // padded leading dimension
-constexpr int OP_BYTES = TW * LDH * 8;  // 34,816
-constexpr int STAGE_BYTES = 2 * OP_BYTES + KH * 8;
-constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
-enum { F_DONE = 1, F_DIAG = 2, F_HALF1 = 4 };
-}  // namespace vx
-
-template <bool GGA>
-__global__ void __launch_bounds__(288, 1)
-    k_vxc(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
-          const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
-          const double* __restrict__ phi, const double* __restrict__ zmat, const double* __restrict__ wv_s, int n_ao,
-          double* __restrict__ Vp) {
-  using namespace vx;
-  extern __shared__ __align__(128) unsigned char smem[];
-  int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
-  const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) {
-    for (int s = 0; s < NST; ++s) {
-      mbar_init(bar0 + 8 * s, 1);
-      mbar_init(bar0 + 8 * (NST + s), 8);
-    }
-    fence_mbar_init();
-  }
-  __syncthreads();
-
-  if (warp == 8) {
-    // ------------------------------------------------------------------ producer warp
-    int s = 0;
-    uint32_t ph = 0;
-    for (;;) {
-      int t = 0;
-      if (lane == 0) t = atomicAdd(ticket, 1);
-      t = __shfl_sync(0xffffffffu, t, 0);
-      if (t >= n_tasks) break;
-      const int p = tasks[t];
-      const int K8 = (kp[p] + 7) & ~7;
-      const int64_t base = panel_off[p];
-      const int nt = (K8 + TW - 1) / TW;
-      const int W = (((K8 + nt - 1) / nt) + 7) & ~7;
-      for (int i = 0; i < nt; ++i) {
-        const int i0 = i * W, wi = min(W, K8 - i0);
-        for (int j = GGA ? 0 : i; j < nt; ++j) {
-          const int j0 = j * W, wj = min(W, K8 - j0);
-          const bool diag = !GGA && (i == j);
-          for (int h = 0; h < 2; ++h) {
-            mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
-            const uint32_t full = bar0 + 8 * s;
-            if (lane == 0) {
-              hdr[4 * s + 0] = p;
-              hdr[4 * s + 1] = i0 | (j0 << 16);
-              hdr[4 * s + 2] = (wi >> 3) | ((wj >> 3) << 8) | (((diag ? F_DIAG : 0) | (h ? F_HALF1 : 0)) << 16);
-              mbar_arrive_expect_tx(full, (uint32_t)((wi + (diag ? 0 : wj)) * (KH * 8) + (GGA ? 0 : KH * 8)));
-            }
-            __syncwarp();
-            const uint32_t sa = smem_u32(smem + s * STAGE_BYTES), sb = sa + OP_BYTES, sw = sb + OP_BYTES;
-            for (int c = lane; c < wi; c += 32)
-              bulk_g2s(sa + c * (LDH * 8), phi + (base + i0 + c) * GB + h * KH, KH * 8, full);
-            if (!diag) {
-              const double* src = GGA ? zmat : phi;
-              for (int c = lane; c < wj; c += 32)
-                bulk_g2s(sb + c * (LDH * 8), src + (base + j0 + c) * GB + h * KH, KH * 8, full);
-            }
-            if (!GGA && lane == 0) bulk_g2s(sw, wv_s + (int64_t)p * GB + h * KH, KH * 8, full);
-            if (++s == NST) { s = 0; ph ^= 1; }
-          }
-        }
-      }
-    }
-    mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
-    if (lane == 0) {
-      hdr[4 * s + 2] = F_DONE << 16;
-      mbar_arrive(bar0 + 8 * s);
-    }
-    return;
-  }
-
-  // -------------------------------------------------------------------- consumer warps: 16 x 32 sub-tiles
-  const int wm = warp & 3, wn = warp >> 2, q4 = lane >> 2, r4 = lane & 3;
-  double acc[2][4][2];
-  int s = 0;
-  uint32_t ph = 0;
-  for (;;) {
-    mbar_wait(bar0 + 8 * s, ph);
-    const int p = hdr[4 * s + 0], ij = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
-    const int fl = h2 >> 16;
-    if (fl & F_DONE) break;
-    const int wi = (h2 & 0xff) << 3, wj = ((h2 >> 8) & 0xff) << 3;
-    if (!(fl & F_HALF1)) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
-    }
-    const int m0 = 16 * wm, nb = 32 * wn;
-    const int nj = min(4, max(0, (wj - nb) >> 3));  // active 8-column sub-tiles of this warp
-    if (m0 < wi && nj > 0) {
-      const bool m1 = (m0 + 8 < wi);
-      const double* As = reinterpret_cast<const double*>(smem + s * STAGE_BYTES);
-      const double* Bs = (fl & F_DIAG) ? As : reinterpret_cast<const double*>(smem + s * STAGE_BYTES + OP_BYTES);
-      const double* ws = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + 2 * OP_BYTES) + r4;
-      const double* pa = As + (m0 + q4) * LDH + r4;
-      const double* pb = Bs + (nb + q4) * LDH + r4;
-#pragma unroll 4
-      for (int ks = 0; ks < KH / 4; ++ks) {
-        double a0 = pa[4 * ks], a1 = m1 ? pa[8 * LDH + 4 * ks] : 0.0;
-        if (!GGA) {
-          const double w = ws[4 * ks];
-          a0 *= w;
-          a1 *= w;
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          if (j < nj) {
-            const double b = pb[j * 8 * LDH + 4 * ks];
-            dmma884(acc[0][j][0], acc[0][j][1], a0, b);
-            if (m1) dmma884(acc[1][j][0], acc[1][j][1], a1, b);
-          }
-        }
-      }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
-    if (++s == NST) { s = 0; ph ^= 1; }
-
-    if (fl & F_HALF1) {
-      // scatter-accumulate the packed tile into the plan-order matrix (upper triangle for LDA)
-      const int K = kp[p];
-      const int64_t base = panel_off[p];
-      const int i0 = ij & 0xffff, j0 = ij >> 16;
-#pragma unroll
-      for (int mi = 0; mi < 2; ++mi) {
-        const int r = i0 + m0 + 8 * mi + q4;
-        if (m0 + 8 * mi < wi && r < K) {
-          const int64_t ci = (int64_t)colidx[base + r] * n_ao;
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            if (j < nj) {
-#pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const int c = j0 + nb + 8 * j + 2 * r4 + e;
-                if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + colidx[base + c], acc[mi][j][e]);
-              }
-            }
-          }
-        }
-      }
-    }
-  }
-}
+// H4 (V contraction) lives in vgram.cu.
 
 // ===================================================================================== H5
 template <bool GGA>
@@ -508,8 +338,6 @@ static kldi_status set_attrs() {
   if (g_attr_done) return KLDI_OK;
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
-  KLDI_CUDA(cudaFuncSetAttribute(k_vxc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
-  KLDI_CUDA(cudaFuncSetAttribute(k_vxc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, vx::SMEM_BYTES));
   g_attr_done = 1;
   return KLDI_OK;
 }
@@ -567,28 +395,6 @@ kldi_status launch_xc(kldi_plan* P, kldi_functional f) {
 kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga) {
   const int nb = (int)((P->n_pad + 255) / 256);
   k_gather_wv<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, gga ? 4 : 1, wv, P->d_wv_s);
-  KLDI_CUDA(cudaGetLastError());
-  return KLDI_OK;
-}
-
-kldi_status launch_vxc(kldi_plan* P, bool gga) {
-  kldi_status rc = set_attrs();
-  if (rc != KLDI_OK) return rc;
-  KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
-  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
-  if (P->n_tasks == 0) return KLDI_OK;
-  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
-  if (gga) {
-    k_build_z<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_kp, P->d_panel_off, P->n_pad, P->d_wv_s, P->d_phi,
-                                                       P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_z);
-    KLDI_CUDA(cudaGetLastError());
-    k_vxc<true><<<grid, 288, vx::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
-                                                          P->d_colidx, P->d_phi, P->d_z, P->d_wv_s, P->n_ao, P->d_Vp);
-  } else {
-    k_vxc<false><<<grid, 288, vx::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
-                                                           P->d_panel_off, P->d_colidx, P->d_phi, nullptr, P->d_wv_s,
-                                                           P->n_ao, P->d_Vp);
-  }
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }

@@ -69,6 +69,17 @@ struct kldi_plan {
   double* d_dphi[3] = {nullptr, nullptr, nullptr};
   double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, same layout as d_phi
 
+  // ---- V contraction schedule (vsched.h), index 0: LDA upper triangle, 1: GGA square
+  int32_t* d_vsched_ptr[2] = {nullptr, nullptr};  // [max_nb + 2] first pass of an nb-block panel
+  void* d_vpasses[2] = {nullptr, nullptr};
+  void* d_vitems[2] = {nullptr, nullptr};
+  int64_t* d_gram_off[2] = {nullptr, nullptr};    // [n_blocks + 1] workspace offsets of G_p (deterministic mode)
+  int64_t gram_elems[2] = {0, 0};
+  double* d_gram = nullptr;                       // lazily allocated workspace of G_p partials
+  int64_t gram_cap = 0;
+  int32_t* d_ao_shell = nullptr;                  // plan AO -> plan shell
+  int v_mode = 0;                                 // 0: red.global.add epilogue, 1: workspace + fixed-order reduce
+
   // ---- task lists
   int32_t* d_tasks = nullptr;  // non-empty grid blocks in Morton order
   int32_t n_tasks = 0;
@@ -101,4 +112,6 @@ kldi_status launch_xc(kldi_plan* P, kldi_functional f);
 kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga);
 kldi_status launch_vxc(kldi_plan* P, bool gga);
 kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V);
+// vgram.cu
+kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const std::vector<int32_t>& h_sh_ao0);
 }  // namespace kldi

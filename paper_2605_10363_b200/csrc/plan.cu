@@ -207,7 +207,9 @@ void plan_free(kldi_plan* P) {
                   P->d_keys, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_col_ptr, P->d_row_idx, P->d_pos,
                   P->d_blk_amax, P->d_panel_off, P->d_kp, P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                   P->d_dphi[2], P->d_z, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
-                  P->d_wv_s, P->d_epart, P->d_E, P->d_stage_host};
+                  P->d_wv_s, P->d_epart, P->d_E, P->d_stage_host, P->d_vsched_ptr[0], P->d_vsched_ptr[1],
+                  P->d_vpasses[0], P->d_vpasses[1], P->d_vitems[0], P->d_vitems[1], P->d_gram_off[0],
+                  P->d_gram_off[1], P->d_gram, P->d_ao_shell};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (P->h_E) cudaFreeHost(P->h_E);
@@ -387,7 +389,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   blk_col0.clear();
   std::vector<int32_t> h_kp(n_blocks), h_colidx, h_tasks;
   std::vector<int32_t> col_cnt(n_shells + 1, 0);
-  double f_rho_u = 0, f_v_u = 0;
+  double f_rho_u = 0, f_v_u = 0, f_rho_us = 0;
   int64_t sum_k = 0, max_k = 0;
   for (int64_t p = 0; p < n_blocks; ++p) {
     const uint8_t* kp = h_keep.data() + (size_t)p * n_shells;
@@ -414,6 +416,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
     sum_k += k;
     max_k = std::max<int64_t>(max_k, k);
     f_rho_u += 2.0 * GB * (double)k * k;
+    f_rho_us += (double)GB * k * (k + 1.0);
     f_v_u += P->want_grad ? 2.0 * GB * (double)k * k : (double)GB * k * (k + 1.0);
   }
   P->total_cols = panel_off[n_blocks];
@@ -449,6 +452,13 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   UP(P->d_colidx, h_colidx);
   UP(P->d_tasks, h_tasks);
   P->n_tasks = (int32_t)h_tasks.size();
+  {
+    const kldi_status rcv = vsched_upload(P, h_kp, h_sh_ao0);
+    if (rcv != KLDI_OK) {
+      cleanup();
+      return rcv;
+    }
+  }
   CK(cudaMalloc(&P->d_blk_amax, sizeof(double) * std::max<int64_t>(1, retained)));
   CK(cudaMemsetAsync(P->d_blk_amax, 0, sizeof(double) * std::max<int64_t>(1, retained), st));
 
@@ -510,6 +520,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   S.workspace_bytes = (int64_t)(2 * nn + sizeof(double) * 8 * n_pad + sizeof(double) * 4 * n_pad +
                                 sizeof(int32_t) * (3 * retained * 2 + P->total_cols));
   S.flops_rho_useful = f_rho_u;
+  S.flops_rho_useful_sym = f_rho_us;
   S.flops_v_useful = f_v_u;
   S.flops_dense = 2.0 * (double)n_pts * n_ao * n_ao;
   S.eps = P->eps;

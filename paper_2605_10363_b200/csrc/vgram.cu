@@ -1,0 +1,311 @@
+// H4: V contraction.  Per grid block p the packed Gram matrix G_p = Phi_p^T diag(wv_p) Phi_p (LDA: strips
+// on and above the diagonal; GGA: B_p = Phi_p^T Z_p, the full square) is formed by FP64 tensor-core MMAs
+// (DMMA.8x8x4) and added to V (Eq. 5/16; accumulate-before-write-back).
+// Persistent, warp-specialised: a producer warp pulls grid blocks from an atomic ticket (on
+// device) and streams 32-row chunks of the panel columns a pass needs through a 3-stage mbarrier ring with
+// bulk-async copies (TMA engine, SASS UBLKCP); 8 consumer warps each hold up to 4 register-resident items
+// (16 rows x <= 32 columns) chosen by the host schedule of vsched.h, so that ragged K_p keeps every warp busy.
+#include "kldi_internal.h"
+#include "ptx.cuh"
+#include "vsched.h"
+
+namespace kldi {
+
+namespace vg {
+constexpr int NST = 3;
+constexpr int RC = 32;              // grid rows (the MMA K dimension) per ring stage
+constexpr int STR = RC + 4;         // padded column stride in doubles: conflict-free 8-B fragment loads
+constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row block of an odd last strip)
+constexpr int COLS_BYTES = NCOL * STR * 8;
+constexpr int STAGE_BYTES = COLS_BYTES + RC * 8;  // + wv chunk
+constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
+enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
+}  // namespace vg
+
+template <int NJ, bool GGA>
+__device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __restrict__ A,
+                                       const double* __restrict__ B, const double* __restrict__ w) {
+  using namespace vg;
+#pragma unroll
+  for (int ks = 0; ks < RC / 4; ++ks) {
+    double a0 = A[4 * ks], a1 = A[8 * STR + 4 * ks];
+    if (!GGA) {
+      const double ww = w[4 * ks];
+      a0 *= ww;
+      a1 *= ww;
+    }
+    double b[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) b[j] = B[j * 8 * STR + 4 * ks];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      dmma884(acc[0][j][0], acc[0][j][1], a0, b[j]);
+      dmma884(acc[1][j][0], acc[1][j][1], a1, b[j]);
+    }
+  }
+}
+
+// ATOMIC = true : the epilogue adds G_p straight into the plan-order V with red.global.add.f64.
+// ATOMIC = false: G_p goes to the workspace (plain 16-B stores) and k_vreduce sums it in a fixed order.
+template <bool GGA, bool ATOMIC>
+__global__ void __launch_bounds__(288, 1)
+    k_vgram(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
+            const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
+            const double* __restrict__ phi, const double* __restrict__ zmat, const double* __restrict__ wv_s,
+            const int32_t* __restrict__ sched_ptr, const VPass* __restrict__ passes, const VItem* __restrict__ items,
+            int n_ao, double* __restrict__ Vp, const int64_t* __restrict__ gram_off, double* __restrict__ G) {
+  using namespace vg;
+  extern __shared__ __align__(128) unsigned char smem[];
+  int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
+  const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);  // full[s] at +8s, empty[s] at +8(NST+s)
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      mbar_init(bar0 + 8 * (NST + s), V_WARPS);
+    }
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  if (warp == V_WARPS) {
+    // ------------------------------------------------------------------ producer warp
+    int s = 0;
+    uint32_t ph = 0;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(ticket, 1);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t >= n_tasks) break;
+      const int p = tasks[t];
+      const int K8 = (kp[p] + 7) & ~7;
+      const int nb = K8 >> 3;
+      const int64_t base = panel_off[p];
+      for (int ps = sched_ptr[nb]; ps < sched_ptr[nb + 1]; ++ps) {
+        const VPass P = passes[ps];
+        const double* src1 = phi + (base + P.c1_lo) * GB;
+        const double* src2 = (GGA ? zmat : phi) + (base + P.c2_lo) * GB;
+        for (int rc = 0; rc < GB / RC; ++rc) {
+          mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+          const uint32_t full = bar0 + 8 * s;
+          if (lane == 0) {
+            hdr[4 * s + 0] = p;
+            hdr[4 * s + 1] = ps;
+            hdr[4 * s + 2] = (rc == 0 ? F_FIRST : 0) | (rc == GB / RC - 1 ? F_LAST : 0);
+            hdr[4 * s + 3] = K8;
+            mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8)));
+          }
+          __syncwarp();
+          const uint32_t sa = smem_u32(smem + s * STAGE_BYTES);
+          for (int c = lane; c < P.c1_n; c += 32)
+            bulk_g2s(sa + c * (STR * 8), src1 + (int64_t)c * GB + rc * RC, RC * 8, full);
+          for (int c = lane; c < P.c2_n; c += 32)
+            bulk_g2s(sa + (P.c1_n + c) * (STR * 8), src2 + (int64_t)c * GB + rc * RC, RC * 8, full);
+          if (!GGA && lane == 0) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
+          if (++s == NST) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+    mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+    if (lane == 0) {
+      hdr[4 * s + 2] = F_DONE;
+      mbar_arrive(bar0 + 8 * s);
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumer warps
+  const int q4 = lane >> 2, r4 = lane & 3;
+  double acc[V_SLOTS][2][4][2];
+  int ia[V_SLOTS], ib[V_SLOTS];
+#pragma unroll
+  for (int k = 0; k < V_SLOTS; ++k) ia[k] = ib[k] = 0;
+  int s = 0;
+  uint32_t ph = 0;
+  for (;;) {
+    mbar_wait(bar0 + 8 * s, ph);
+    const int p = hdr[4 * s + 0], ps = hdr[4 * s + 1], fl = hdr[4 * s + 2], K8 = hdr[4 * s + 3];
+    if (fl & F_DONE) break;
+    if (fl & F_FIRST) {
+      const VItem* it = items + ((int64_t)ps * V_WARPS + warp) * V_SLOTS;
+#pragma unroll
+      for (int k = 0; k < V_SLOTS; ++k) {
+        ia[k] = __ldg(&it[k].a);
+        ib[k] = __ldg(&it[k].b);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[k][0][j][0] = acc[k][0][j][1] = acc[k][1][j][0] = acc[k][1][j][1] = 0.0;
+      }
+    }
+    const double* st = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + q4 * STR + r4;
+    const double* wb = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + COLS_BYTES) + r4;
+#pragma unroll
+    for (int k = 0; k < V_SLOTS; ++k) {
+      const int nj = ia[k] >> 20;
+      const double* A = st + (ia[k] & 1023) * STR;
+      const double* B = st + ((ia[k] >> 10) & 1023) * STR;
+      switch (nj) {
+        case 1: vg_run<1, GGA>(acc[k], A, B, wb); break;
+        case 2: vg_run<2, GGA>(acc[k], A, B, wb); break;
+        case 3: vg_run<3, GGA>(acc[k], A, B, wb); break;
+        case 4: vg_run<4, GGA>(acc[k], A, B, wb); break;
+        default: break;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    if (++s == NST) { s = 0; ph ^= 1; }
+
+    if (fl & F_LAST) {
+      const int K = kp[p];
+      const int64_t base = panel_off[p];
+#pragma unroll
+      for (int k = 0; k < V_SLOTS; ++k) {
+        const int nj = ia[k] >> 20;
+        if (nj == 0) continue;
+        const int arow = ib[k] & 0xffff, bcol = ib[k] >> 16;
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi) {
+          const int r = arow + 8 * mi + q4;
+          if (ATOMIC) {
+            if (r < K) {
+              const int64_t ci = (int64_t)colidx[base + r] * n_ao;
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (j < nj) {
+#pragma unroll
+                  for (int e = 0; e < 2; ++e) {
+                    const int c = bcol + 8 * j + 2 * r4 + e;
+                    if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + colidx[base + c], acc[k][mi][j][e]);
+                  }
+                }
+            }
+          } else {
+            if (arow + 8 * mi < K8) {
+              // LDA: strip-packed upper triangle (strip s: 16 rows x (K8 - 16 s) columns); GGA: K8 x K8 square
+              const int sx = arow >> 4;
+              const int64_t rowoff = GGA ? (int64_t)r * K8
+                                         : (int64_t)16 * sx * K8 - (int64_t)128 * sx * (sx - 1) +
+                                               (int64_t)(8 * mi + q4) * (K8 - 16 * sx) - 16 * sx;
+              double* g = G + gram_off[p] + rowoff + bcol + 2 * r4;
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (j < nj) *reinterpret_cast<double2*>(g + 8 * j) = make_double2(acc[k][mi][j][0], acc[k][mi][j][1]);
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+// ===================================================================================== host side
+template <typename T>
+static kldi_status up(T** dst, const std::vector<T>& v, cudaStream_t st) {
+  KLDI_CUDA(cudaMalloc((void**)dst, std::max<size_t>(1, v.size()) * sizeof(T)));
+  if (!v.empty()) KLDI_CUDA(cudaMemcpyAsync(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+  return KLDI_OK;
+}
+
+// Builds the pass/item tables for every panel size that occurs, the G_p workspace offsets and the
+// issued-FLOP count of the V kernel (plan stage, once per geometry).
+kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const std::vector<int32_t>& h_sh_ao0) {
+  int max_nb = 0;
+  for (int32_t k : h_kp) max_nb = std::max(max_nb, (k + 7) >> 3);
+  std::vector<int64_t> count(max_nb + 1, 0);
+  for (int32_t k : h_kp) count[(k + 7) >> 3]++;
+  kldi_status rc;
+  for (int m = 0; m < (P->want_grad ? 2 : 1); ++m) {
+    std::vector<int32_t> ptr(max_nb + 2, 0);
+    std::vector<VPass> passes;
+    std::vector<VItem> items;
+    double fexec = 0, fcrit = 0;
+    for (int nb = 0; nb <= max_nb; ++nb) {
+      ptr[nb] = (int32_t)passes.size();
+      if (nb == 0 || count[nb] == 0) continue;
+      vsched_build(nb, m == 1, passes, items);
+      for (size_t i = ptr[nb]; i < passes.size(); ++i) {
+        fexec += (double)count[nb] * passes[i].units * (2.0 * 16 * 8 * GB);
+        fcrit += (double)count[nb] * passes[i].max_load * V_WARPS * (2.0 * 16 * 8 * GB);
+      }
+    }
+    ptr[max_nb + 1] = (int32_t)passes.size();
+    if ((rc = up(&P->d_vsched_ptr[m], ptr, P->stream)) != KLDI_OK) return rc;
+    VPass* dp = nullptr;
+    VItem* di = nullptr;
+    if ((rc = up(&dp, passes, P->stream)) != KLDI_OK) return rc;
+    P->d_vpasses[m] = dp;
+    if ((rc = up(&di, items, P->stream)) != KLDI_OK) return rc;
+    P->d_vitems[m] = di;
+    // workspace offsets of G_p: LDA strip-packed triangle, GGA square
+    std::vector<int64_t> goff(h_kp.size() + 1, 0);
+    for (size_t p = 0; p < h_kp.size(); ++p) {
+      const int64_t k8 = (h_kp[p] + 7) & ~7, ns = (k8 + 15) / 16;
+      goff[p + 1] = goff[p] + (m == 1 ? k8 * k8 : 16 * ns * k8 - 128 * ns * (ns - 1));
+    }
+    P->gram_elems[m] = goff.back();
+    if ((rc = up(&P->d_gram_off[m], goff, P->stream)) != KLDI_OK) return rc;
+    if (m == (P->want_grad ? 1 : 0)) {
+      P->stats.flops_v_exec = fexec;
+      P->stats.flops_v_crit = fcrit;
+    }
+  }
+  std::vector<int32_t> ao_shell;
+  for (size_t s = 0; s + 1 < h_sh_ao0.size(); ++s)
+    for (int c = h_sh_ao0[s]; c < h_sh_ao0[s + 1]; ++c) ao_shell.push_back((int32_t)s);
+  if ((rc = up(&P->d_ao_shell, ao_shell, P->stream)) != KLDI_OK) return rc;
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));  // the host vectors go out of scope
+  return KLDI_OK;
+}
+
+// GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi on the stored tiles (same layout as Phi); HBM-bound.
+__global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off,
+                                                 int64_t n_pad, const double* __restrict__ wv_s,
+                                                 const double* __restrict__ phi, const double* __restrict__ d0,
+                                                 const double* __restrict__ d1, const double* __restrict__ d2,
+                                                 double* __restrict__ z) {
+  const int p = blockIdx.x, t = threadIdx.x;
+  const int64_t g = (int64_t)p * GB + t;
+  const double w0 = 0.5 * wv_s[g], w1 = wv_s[n_pad + g], w2 = wv_s[2 * n_pad + g], w3 = wv_s[3 * n_pad + g];
+  const int64_t o0 = panel_off[p] * GB + t;
+  const int K = kp[p];
+  for (int k = 0; k < K; ++k) {
+    const int64_t o = o0 + (int64_t)k * GB;
+    z[o] = w0 * phi[o] + w1 * d0[o] + w2 * d1[o] + w3 * d2[o];
+  }
+}
+
+template <bool GGA, bool ATOMIC>
+static kldi_status launch_vgram(kldi_plan* P) {
+  static bool attr_done = false;
+  if (!attr_done) {
+    KLDI_CUDA(cudaFuncSetAttribute(k_vgram<GGA, ATOMIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, vg::SMEM_BYTES));
+    attr_done = true;
+  }
+  const int m = GGA ? 1 : 0;
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  k_vgram<GGA, ATOMIC><<<grid, 32 * (V_WARPS + 1), vg::SMEM_BYTES, P->stream>>>(
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi, P->d_z, P->d_wv_s,
+      P->d_vsched_ptr[m], static_cast<const VPass*>(P->d_vpasses[m]), static_cast<const VItem*>(P->d_vitems[m]),
+      P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_vxc(kldi_plan* P, bool gga) {
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->v_mode == 0) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+  if (P->n_tasks == 0) {
+    if (P->v_mode != 0) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+    return KLDI_OK;
+  }
+  if (gga) {
+    k_build_z<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_kp, P->d_panel_off, P->n_pad, P->d_wv_s, P->d_phi,
+                                                       P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_z);
+    KLDI_CUDA(cudaGetLastError());
+  }
+  if (P->v_mode == 0) return gga ? launch_vgram<true, true>(P) : launch_vgram<false, true>(P);
+  set_error("launch_vxc: deterministic V mode not built yet");
+  return KLDI_ESTATE;
+}
+
+}  // namespace kldi
