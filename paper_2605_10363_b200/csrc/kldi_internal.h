@@ -14,6 +14,15 @@ constexpr int GB = 128;  // points per grid block (BASELINE.json; PAPER.md:118 u
 
 void set_error(const char* fmt, ...);
 
+// "V layout" of a panel (second copy of Phi, and Z, read by the V contraction): 4 slabs of 32 grid rows; slab
+// rc holds [K8 columns][32 rows] contiguously, so any column interval of a slab is ONE bulk copy; inside a
+// column the 16-byte chunk c (rows 2c, 2c+1) sits at chunk c ^ (col & 7), which makes the 16-byte MMA
+// fragment loads of 8 adjacent columns bank-conflict free without padding (the smem image is the HBM image).
+__host__ __device__ __forceinline__ int64_t vlayout_off(int64_t panel_off_p, int K8, int col, int row) {
+  const int rc = row >> 5, rr = row & 31, c = rr >> 1;
+  return panel_off_p * GB + (int64_t)rc * K8 * 32 + (int64_t)col * 32 + (((c ^ (col & 7)) << 1) | (rr & 1));
+}
+
 #define KLDI_CUDA(call)                                                                     \
   do {                                                                                      \
     cudaError_t e__ = (call);                                                               \
@@ -67,7 +76,8 @@ struct kldi_plan {
   int64_t total_cols = 0;
   double* d_phi = nullptr;         // [total_cols + slack][128] column-major tiles
   double* d_dphi[3] = {nullptr, nullptr, nullptr};
-  double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, same layout as d_phi
+  double* d_phi_v = nullptr;       // second copy of Phi in the V layout (vlayout_off)
+  double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, V layout
 
   // ---- V contraction schedule (vsched.h), index 0: LDA upper triangle, 1: GGA square
   int32_t* d_vsched_ptr[2] = {nullptr, nullptr};  // [max_nb + 2] first pass of an nb-block panel

@@ -161,13 +161,14 @@ __global__ void __launch_bounds__(128) k_fill(ShellTable T, const int32_t* __res
                                               const int32_t* __restrict__ blk_col0,
                                               const int64_t* __restrict__ panel_off, const double* __restrict__ gx,
                                               const double* __restrict__ gy, const double* __restrict__ gz,
-                                              double* __restrict__ phi, double* __restrict__ d0,
-                                              double* __restrict__ d1, double* __restrict__ d2,
-                                              unsigned long long* __restrict__ amax_bits) {
+                                              double* __restrict__ phi, double* __restrict__ phi_v,
+                                              double* __restrict__ d0, double* __restrict__ d1,
+                                              double* __restrict__ d2, unsigned long long* __restrict__ amax_bits) {
   const int p = blockIdx.x, t = threadIdx.x, lane = t & 31;
   const int64_t g = (int64_t)p * GB + t;
   const double x = gx[g], y = gy[g], z = gz[g];
   const int64_t base = panel_off[p] * GB + t;
+  const int K8 = (int)(panel_off[p + 1] - panel_off[p]);
   for (int e = row_ptr[p]; e < row_ptr[p + 1]; ++e) {
     const int s = col_idx[e];
     const int l = T.sh_l[s];
@@ -178,6 +179,7 @@ __global__ void __launch_bounds__(128) k_fill(ShellTable T, const int32_t* __res
     double m = 0.0;
     for (int c = 0; c < nc; ++c) {
       phi[o + (int64_t)c * GB] = val[c];
+      phi_v[vlayout_off(panel_off[p], K8, blk_col0[e] + c, t)] = val[c];
       m = fmax(m, fabs(val[c]));
       if (GRAD) {
         d0[o + (int64_t)c * GB] = g0[c];
@@ -206,7 +208,7 @@ void plan_free(kldi_plan* P) {
                   P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
                   P->d_keys, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_col_ptr, P->d_row_idx, P->d_pos,
                   P->d_blk_amax, P->d_panel_off, P->d_kp, P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
-                  P->d_dphi[2], P->d_z, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
+                  P->d_dphi[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
                   P->d_wv_s, P->d_epart, P->d_E, P->d_stage_host, P->d_vsched_ptr[0], P->d_vsched_ptr[1],
                   P->d_vpasses[0], P->d_vpasses[1], P->d_vitems[0], P->d_vitems[1], P->d_gram_off[0],
                   P->d_gram_off[1], P->d_gram, P->d_ao_shell};
@@ -466,7 +468,9 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   const size_t tile_bytes = sizeof(double) * GB * (size_t)(P->total_cols + 64);
   CK(cudaMalloc(&P->d_phi, tile_bytes));
   CK(cudaMemsetAsync(P->d_phi, 0, tile_bytes, st));
-  int64_t phi_bytes = (int64_t)tile_bytes;
+  CK(cudaMalloc(&P->d_phi_v, tile_bytes));
+  CK(cudaMemsetAsync(P->d_phi_v, 0, tile_bytes, st));
+  int64_t phi_bytes = 2 * (int64_t)tile_bytes;
   if (P->want_grad) {
     for (int c = 0; c < 3; ++c) {
       CK(cudaMalloc(&P->d_dphi[c], tile_bytes));
@@ -474,15 +478,15 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
     }
     CK(cudaMalloc(&P->d_z, tile_bytes));
     CK(cudaMemsetAsync(P->d_z, 0, tile_bytes, st));
-    phi_bytes *= 5;
+    phi_bytes += 4 * (int64_t)tile_bytes;
   }
   if (P->want_grad)
     k_fill<true><<<(int)n_blocks, 128, 0, st>>>(T, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_panel_off, P->d_gx,
-                                                P->d_gy, P->d_gz, P->d_phi, P->d_dphi[0], P->d_dphi[1], P->d_dphi[2],
+                                                P->d_gy, P->d_gz, P->d_phi, P->d_phi_v, P->d_dphi[0], P->d_dphi[1], P->d_dphi[2],
                                                 (unsigned long long*)P->d_blk_amax);
   else
     k_fill<false><<<(int)n_blocks, 128, 0, st>>>(T, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_panel_off,
-                                                 P->d_gx, P->d_gy, P->d_gz, P->d_phi, nullptr, nullptr, nullptr,
+                                                 P->d_gx, P->d_gy, P->d_gz, P->d_phi, P->d_phi_v, nullptr, nullptr, nullptr,
                                                  (unsigned long long*)P->d_blk_amax);
   CK(cudaGetLastError());
 

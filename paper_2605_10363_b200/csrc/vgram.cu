@@ -13,8 +13,8 @@ namespace kldi {
 
 namespace vg {
 constexpr int NST = 3;
-constexpr int RC = 32;              // grid rows (the MMA K dimension) per ring stage
-constexpr int STR = RC + 4;         // padded column stride in doubles: conflict-free 8-B fragment loads
+constexpr int RC = 32;              // grid rows (the MMA K dimension) per ring stage = one slab of the V layout
+constexpr int STR = RC;             // column stride in doubles: dense, the chunk swizzle of vlayout_off avoids conflicts
 constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row block of an odd last strip)
 constexpr int COLS_BYTES = NCOL * STR * 8;
 constexpr int STAGE_BYTES = COLS_BYTES + RC * 8;  // + wv chunk
@@ -22,25 +22,37 @@ constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
 enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
 }  // namespace vg
 
+// One slab (32 grid rows = 8 k-steps) of one item.  A, B point at the item's first column (+ q4 columns);
+// o0/o1 are the lane's swizzled offsets of chunks 2 r4 and 2 r4 + 1; a 16-byte load feeds two k-steps.
 template <int NJ, bool GGA>
 __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __restrict__ A,
-                                       const double* __restrict__ B, const double* __restrict__ w) {
+                                       const double* __restrict__ B, const double* __restrict__ w, int o0, int o1) {
   using namespace vg;
 #pragma unroll
-  for (int ks = 0; ks < RC / 4; ++ks) {
-    double a0 = A[4 * ks], a1 = A[8 * STR + 4 * ks];
-    if (!GGA) {
-      const double ww = w[4 * ks];
-      a0 *= ww;
-      a1 *= ww;
-    }
-    double b[NJ];
+  for (int h = 0; h < 2; ++h) {
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) b[j] = B[j * 8 * STR + 4 * ks];
+    for (int j = 0; j < 2; ++j) {
+      const int o = (j ? o1 : o0) + 16 * h;
+      double2 a0 = *reinterpret_cast<const double2*>(A + o);
+      double2 a1 = *reinterpret_cast<const double2*>(A + 8 * STR + o);
+      if (!GGA) {
+        const double2 ww = *reinterpret_cast<const double2*>(w + 2 * j + 16 * h);
+        a0.x *= ww.x; a0.y *= ww.y;
+        a1.x *= ww.x; a1.y *= ww.y;
+      }
+      double2 b[NJ];
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-      dmma884(acc[0][j][0], acc[0][j][1], a0, b[j]);
-      dmma884(acc[1][j][0], acc[1][j][1], a1, b[j]);
+      for (int n = 0; n < NJ; ++n) b[n] = *reinterpret_cast<const double2*>(B + n * 8 * STR + o);
+#pragma unroll
+      for (int n = 0; n < NJ; ++n) {
+        dmma884(acc[0][n][0], acc[0][n][1], a0.x, b[n].x);
+        dmma884(acc[1][n][0], acc[1][n][1], a1.x, b[n].x);
+      }
+#pragma unroll
+      for (int n = 0; n < NJ; ++n) {
+        dmma884(acc[0][n][0], acc[0][n][1], a0.y, b[n].y);
+        dmma884(acc[1][n][0], acc[1][n][1], a1.y, b[n].y);
+      }
     }
   }
 }
@@ -83,8 +95,6 @@ __global__ void __launch_bounds__(288, 1)
       const int64_t base = panel_off[p];
       for (int ps = sched_ptr[nb]; ps < sched_ptr[nb + 1]; ++ps) {
         const VPass P = passes[ps];
-        const double* src1 = phi + (base + P.c1_lo) * GB;
-        const double* src2 = (GGA ? zmat : phi) + (base + P.c2_lo) * GB;
         for (int rc = 0; rc < GB / RC; ++rc) {
           mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
           const uint32_t full = bar0 + 8 * s;
@@ -96,12 +106,15 @@ __global__ void __launch_bounds__(288, 1)
             mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8)));
           }
           __syncwarp();
-          const uint32_t sa = smem_u32(smem + s * STAGE_BYTES);
-          for (int c = lane; c < P.c1_n; c += 32)
-            bulk_g2s(sa + c * (STR * 8), src1 + (int64_t)c * GB + rc * RC, RC * 8, full);
-          for (int c = lane; c < P.c2_n; c += 32)
-            bulk_g2s(sa + (P.c1_n + c) * (STR * 8), src2 + (int64_t)c * GB + rc * RC, RC * 8, full);
-          if (!GGA && lane == 0) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
+          if (lane == 0) {  // one bulk copy per column interval: the slab is contiguous in the V layout
+            const uint32_t sa = smem_u32(smem + s * STAGE_BYTES);
+            const int64_t slab = base * GB + (int64_t)rc * K8 * RC;
+            bulk_g2s(sa, phi + slab + (int64_t)P.c1_lo * RC, (uint32_t)P.c1_n * (RC * 8), full);
+            if (P.c2_n)
+              bulk_g2s(sa + P.c1_n * (RC * 8), (GGA ? zmat : phi) + slab + (int64_t)P.c2_lo * RC,
+                       (uint32_t)P.c2_n * (RC * 8), full);
+            if (!GGA) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
+          }
           if (++s == NST) { s = 0; ph ^= 1; }
         }
       }
@@ -116,6 +129,7 @@ __global__ void __launch_bounds__(288, 1)
 
   // -------------------------------------------------------------------- consumer warps
   const int q4 = lane >> 2, r4 = lane & 3;
+  const int o0 = ((2 * r4) ^ q4) * 2, o1 = ((2 * r4 + 1) ^ q4) * 2;  // swizzled chunk offsets (doubles)
   double acc[V_SLOTS][2][4][2];
   int ia[V_SLOTS], ib[V_SLOTS];
 #pragma unroll
@@ -136,18 +150,18 @@ __global__ void __launch_bounds__(288, 1)
         for (int j = 0; j < 4; ++j) acc[k][0][j][0] = acc[k][0][j][1] = acc[k][1][j][0] = acc[k][1][j][1] = 0.0;
       }
     }
-    const double* st = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + q4 * STR + r4;
-    const double* wb = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + COLS_BYTES) + r4;
+    const double* st = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + q4 * STR;
+    const double* wb = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + COLS_BYTES) + 4 * r4;
 #pragma unroll
     for (int k = 0; k < V_SLOTS; ++k) {
       const int nj = ia[k] >> 20;
       const double* A = st + (ia[k] & 1023) * STR;
       const double* B = st + ((ia[k] >> 10) & 1023) * STR;
       switch (nj) {
-        case 1: vg_run<1, GGA>(acc[k], A, B, wb); break;
-        case 2: vg_run<2, GGA>(acc[k], A, B, wb); break;
-        case 3: vg_run<3, GGA>(acc[k], A, B, wb); break;
-        case 4: vg_run<4, GGA>(acc[k], A, B, wb); break;
+        case 1: vg_run<1, GGA>(acc[k], A, B, wb, o0, o1); break;
+        case 2: vg_run<2, GGA>(acc[k], A, B, wb, o0, o1); break;
+        case 3: vg_run<3, GGA>(acc[k], A, B, wb, o0, o1); break;
+        case 4: vg_run<4, GGA>(acc[k], A, B, wb, o0, o1); break;
         default: break;
       }
     }
@@ -257,7 +271,7 @@ kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const 
   return KLDI_OK;
 }
 
-// GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi on the stored tiles (same layout as Phi); HBM-bound.
+// GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi from the stored tiles, written in the V layout; HBM-bound.
 __global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off,
                                                  int64_t n_pad, const double* __restrict__ wv_s,
                                                  const double* __restrict__ phi, const double* __restrict__ d0,
@@ -267,10 +281,10 @@ __global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp,
   const int64_t g = (int64_t)p * GB + t;
   const double w0 = 0.5 * wv_s[g], w1 = wv_s[n_pad + g], w2 = wv_s[2 * n_pad + g], w3 = wv_s[3 * n_pad + g];
   const int64_t o0 = panel_off[p] * GB + t;
-  const int K = kp[p];
+  const int K = kp[p], K8 = (K + 7) & ~7;
   for (int k = 0; k < K; ++k) {
     const int64_t o = o0 + (int64_t)k * GB;
-    z[o] = w0 * phi[o] + w1 * d0[o] + w2 * d1[o] + w3 * d2[o];
+    z[vlayout_off(panel_off[p], K8, k, t)] = w0 * phi[o] + w1 * d0[o] + w2 * d1[o] + w3 * d2[o];
   }
 }
 
@@ -284,7 +298,7 @@ static kldi_status launch_vgram(kldi_plan* P) {
   const int m = GGA ? 1 : 0;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   k_vgram<GGA, ATOMIC><<<grid, 32 * (V_WARPS + 1), vg::SMEM_BYTES, P->stream>>>(
-      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi, P->d_z, P->d_wv_s,
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi_v, P->d_z, P->d_wv_s,
       P->d_vsched_ptr[m], static_cast<const VPass*>(P->d_vpasses[m]), static_cast<const VItem*>(P->d_vitems[m]),
       P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram);
   KLDI_CUDA(cudaGetLastError());
