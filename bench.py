@@ -153,6 +153,8 @@ def main():
     ap.add_argument("--eps", type=float, default=1e-12)
     ap.add_argument("--ref-sample", type=int, default=4096)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1],
+                    help="1: V without FP64 atomics (workspace partials + fixed-order reduce)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "kldi" else args.warmup
 
@@ -190,6 +192,7 @@ def main():
     gga = wl.functional == "gga"
     func = K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER
     plan = K.Plan.from_workload(wl)
+    plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
     st = plan.stats.as_dict()
     D = torch.as_tensor(wl.D, device="cuda")
     V = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")

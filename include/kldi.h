@@ -163,6 +163,13 @@ kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_
 kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, double* out,
                                   int64_t cap_bytes, int32_t* width);
 
+/* Options of a plan.  KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram
+ * tile into V with red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a
+ * workspace (allocated on first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed
+ * order: no FP64 atomics, V bitwise reproducible.  Returns KLDI_EINVAL for unknown options. */
+typedef enum { KLDI_OPT_DETERMINISTIC_V = 1 } kldi_option;
+kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
+
 /* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`
  * iterations; returns achieved TFLOP/s (device-timed) in *tflops.  kind 0 = DMMA, 1 = DFMA. */
 kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);

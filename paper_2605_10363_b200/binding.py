@@ -21,8 +21,9 @@ KLDI_GGA_PBEX = 1
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
-    "kldi_morton_key", "kldi_last_error",
+    "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option",
 ]
+KLDI_OPT_DETERMINISTIC_V = 1
 
 
 class KldiError(RuntimeError):
@@ -179,6 +180,9 @@ class Plan:
         _check(lib().kldi_build_vxc(self._h, self._dev64(wv, shape, "wv"), 1 if gga else 0,
                                     self._dev64(V, (self.n_ao, self.n_ao), "V")), "kldi_build_vxc")
         return V
+
+    def set_option(self, option: int, value: int):
+        _check(lib().kldi_plan_set_option(self._h, int(option), int(value)), "kldi_plan_set_option")
 
     def exc(self, D, functional: int = KLDI_LDA_SLATER, out=None, want_v: bool = True):
         import torch

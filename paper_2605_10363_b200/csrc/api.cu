@@ -245,6 +245,15 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
   return KLDI_OK;
 }
 
+kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
+  if (!P || option != KLDI_OPT_DETERMINISTIC_V) {
+    set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);
+    return KLDI_EINVAL;
+  }
+  P->v_mode = value ? 1 : 0;
+  return KLDI_OK;
+}
+
 kldi_status kldi_last_timings(kldi_plan* P, double* out) {
   if (!P || !out) {
     set_error("kldi_last_timings: null argument");

@@ -305,6 +305,78 @@ static kldi_status launch_vgram(kldi_plan* P) {
   return KLDI_OK;
 }
 
+// ===================================================================================== H5a fixed-order reduce
+// Deterministic mode: V[i, :] = sum over the grid blocks p that retain AO i (BCS(C) column of its shell,
+// ascending p: PAPER.md:466-470) of row r_p(i) of G_p, scattered through colidx.  One warp per plan AO row, the
+// row accumulated in shared memory in that fixed order: no atomics, bitwise reproducible ("partial sums
+// contributing to the same output tile are accumulated before the final write-back").
+template <bool GGA>
+__global__ void __launch_bounds__(128) k_vreduce(int n_ao, const int32_t* __restrict__ ao_shell,
+                                                 const int32_t* __restrict__ sh_ao0, const int32_t* __restrict__ col_ptr,
+                                                 const int32_t* __restrict__ row_idx, const int32_t* __restrict__ pos,
+                                                 const int32_t* __restrict__ blk_col0, const int32_t* __restrict__ kp,
+                                                 const int64_t* __restrict__ panel_off,
+                                                 const int64_t* __restrict__ gram_off,
+                                                 const int32_t* __restrict__ colidx, const double* __restrict__ G,
+                                                 double* __restrict__ Vp) {
+  extern __shared__ double rowbuf[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int i = blockIdx.x * (blockDim.x >> 5) + warp;
+  if (i >= n_ao) return;
+  double* buf = rowbuf + (size_t)warp * n_ao;
+  for (int j = lane; j < n_ao; j += 32) buf[j] = 0.0;
+  __syncwarp();
+  const int q = ao_shell[i], a = i - sh_ao0[q];
+  const int e_end = col_ptr[q + 1];
+  for (int e0 = col_ptr[q]; e0 < e_end; e0 += 32) {
+    // lane-parallel metadata of up to 32 contributions
+    int64_t m_row = 0, m_base = 0;
+    int m_c0 = 0, m_K = 0;
+    if (e0 + lane < e_end) {
+      const int p = row_idx[e0 + lane];
+      const int r = blk_col0[pos[e0 + lane]] + a;
+      m_K = kp[p];
+      const int K8 = (m_K + 7) & ~7;
+      m_base = panel_off[p];
+      if (GGA) {
+        m_row = gram_off[p] + (int64_t)r * K8;
+        m_c0 = 0;
+      } else {
+        const int sx = r >> 4;
+        m_row = gram_off[p] + (int64_t)16 * sx * K8 - (int64_t)128 * sx * (sx - 1) +
+                (int64_t)(r - 16 * sx) * (K8 - 16 * sx) - 16 * sx;
+        m_c0 = r;
+      }
+    }
+    const int n = min(32, e_end - e0);
+    for (int t = 0; t < n; ++t) {
+      const int64_t row = __shfl_sync(0xffffffffu, m_row, t), base = __shfl_sync(0xffffffffu, m_base, t);
+      const int c0 = __shfl_sync(0xffffffffu, m_c0, t), K = __shfl_sync(0xffffffffu, m_K, t);
+      for (int c = c0 + lane; c < K; c += 32) buf[colidx[base + c]] += G[row + c];
+      __syncwarp();
+    }
+  }
+  for (int j = (GGA ? 0 : i) + lane; j < n_ao; j += 32) Vp[(int64_t)i * n_ao + j] = buf[j];
+}
+
+template <bool GGA>
+static kldi_status launch_vreduce(kldi_plan* P) {
+  const size_t row_bytes = sizeof(double) * (size_t)P->n_ao;
+  int wpb = (int)std::min<size_t>(4, (220 * 1024) / row_bytes);
+  if (wpb < 1) {
+    set_error("deterministic V mode: n_ao = %d exceeds the shared-memory row buffer (28160)", P->n_ao);
+    return KLDI_EINVAL;
+  }
+  const size_t smem = wpb * row_bytes;
+  KLDI_CUDA(cudaFuncSetAttribute(k_vreduce<GGA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int m = GGA ? 1 : 0;
+  k_vreduce<GGA><<<(P->n_ao + wpb - 1) / wpb, 32 * wpb, smem, P->stream>>>(
+      P->n_ao, P->d_ao_shell, P->d_sh_ao0, P->d_col_ptr, P->d_row_idx, P->d_pos, P->d_blk_col0, P->d_kp,
+      P->d_panel_off, P->d_gram_off[m], P->d_colidx, P->d_gram, P->d_Vp);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
 kldi_status launch_vxc(kldi_plan* P, bool gga) {
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
   if (P->v_mode == 0) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
@@ -318,8 +390,18 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
     KLDI_CUDA(cudaGetLastError());
   }
   if (P->v_mode == 0) return gga ? launch_vgram<true, true>(P) : launch_vgram<false, true>(P);
-  set_error("launch_vxc: deterministic V mode not built yet");
-  return KLDI_ESTATE;
+  // deterministic mode: G_p partials to the workspace, then the fixed-order reduce
+  const int m = gga ? 1 : 0;
+  if (P->gram_cap < P->gram_elems[m]) {
+    if (P->d_gram) KLDI_CUDA(cudaFree(P->d_gram));
+    P->d_gram = nullptr;
+    P->gram_cap = 0;
+    KLDI_CUDA(cudaMalloc(&P->d_gram, sizeof(double) * (size_t)std::max<int64_t>(1, P->gram_elems[m])));
+    P->gram_cap = P->gram_elems[m];
+  }
+  kldi_status rc = gga ? launch_vgram<true, false>(P) : launch_vgram<false, false>(P);
+  if (rc != KLDI_OK) return rc;
+  return gga ? launch_vreduce<true>(P) : launch_vreduce<false>(P);
 }
 
 }  // namespace kldi

@@ -28,11 +28,12 @@ def K():
     return binding
 
 
-def run_gpu(K, wl, eps=None):
+def run_gpu(K, wl, eps=None, deterministic_v=0):
     import torch
 
     gga = wl.functional == "gga"
     plan = K.Plan.from_workload(wl, eps=eps)
+    plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, deterministic_v)
     D = torch.as_tensor(wl.D, device="cuda")
     E, V = plan.exc(D, K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER)
     if gga:
@@ -299,6 +300,26 @@ def test_reproducible_rho_and_energy(K):
     r2 = plan.eval_rho(D)
     assert E1 == E2 and torch.equal(r1, r2)
     assert float((V1 - V2).abs().max()) <= 1e-14 * float(V1.abs().max())
+    plan.close()
+
+
+@pytest.mark.parametrize("name,n,fn", [("cfg1", 8, "lda"), ("cfg4", 6, "gga"), ("cfg0", None, "lda")])
+def test_deterministic_v_mode(K, name, n, fn):
+    """KLDI_OPT_DETERMINISTIC_V: Gram partials in a workspace + fixed-order reduce (no FP64 atomics):
+    same parity bar, and V bitwise identical between calls."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional=fn)
+    out = run_gpu(K, wl, deterministic_v=1)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, fn)
+    check(out, ref)
+    plan = out["plan"]
+    D = torch.as_tensor(wl.D, device="cuda")
+    f = K.KLDI_GGA_PBEX if fn == "gga" else K.KLDI_LDA_SLATER
+    E1, V1 = plan.exc(D, f)
+    V1 = V1.clone()
+    E2, V2 = plan.exc(D, f)
+    assert E1 == E2 and torch.equal(V1, V2)
     plan.close()
 
 
