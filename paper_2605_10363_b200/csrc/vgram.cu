@@ -349,11 +349,36 @@ __global__ void __launch_bounds__(128) k_vreduce(int n_ao, const int32_t* __rest
       }
     }
     const int n = min(32, e_end - e0);
-    for (int t = 0; t < n; ++t) {
-      const int64_t row = __shfl_sync(0xffffffffu, m_row, t), base = __shfl_sync(0xffffffffu, m_base, t);
-      const int c0 = __shfl_sync(0xffffffffu, m_c0, t), K = __shfl_sync(0xffffffffu, m_K, t);
-      for (int c = c0 + lane; c < K; c += 32) buf[colidx[base + c]] += G[row + c];
-      __syncwarp();
+    // 4 contributions at a time: all their loads are issued before the first dependent shared-memory add, so
+    // one memory latency is paid per group instead of per contribution; the adds stay in ascending-p order.
+    constexpr int NU = 4, NCH = 3;
+    for (int t0 = 0; t0 < n; t0 += NU) {
+      int64_t row[NU], base[NU];
+      int c0[NU], K[NU], jj[NU][NCH];
+      double vv[NU][NCH];
+#pragma unroll
+      for (int u = 0; u < NU; ++u) {
+        const int t = min(t0 + u, 31);
+        row[u] = __shfl_sync(0xffffffffu, m_row, t);
+        base[u] = __shfl_sync(0xffffffffu, m_base, t);
+        c0[u] = __shfl_sync(0xffffffffu, m_c0, t);
+        K[u] = (t0 + u < n) ? __shfl_sync(0xffffffffu, m_K, t) : 0;
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+          const int c = c0[u] + lane + 32 * ch;
+          const bool ok = c < K[u];
+          jj[u][ch] = ok ? __ldg(colidx + base[u] + c) : -1;
+          vv[u][ch] = ok ? __ldcs(G + row[u] + c) : 0.0;
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < NU; ++u) {
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch)
+          if (jj[u][ch] >= 0) buf[jj[u][ch]] += vv[u][ch];
+        for (int c = c0[u] + lane + 32 * NCH; c < K[u]; c += 32) buf[colidx[base[u] + c]] += G[row[u] + c];
+        __syncwarp();
+      }
     }
   }
   for (int j = (GGA ? 0 : i) + lane; j < n_ao; j += 32) Vp[(int64_t)i * n_ao + j] = buf[j];
