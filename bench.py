@@ -256,8 +256,13 @@ def main():
         dmma_live = K.fp64_peak("dmma", 20000)
     except Exception:
         dmma_live = None
-    f_rho, f_v = st["flops_rho_useful"], st["flops_v_useful"]
+    # LDA: the rho build uses D = D^T (triangular D'), so its useful work is 128 K(K+1) per block;
+    # GGA needs the full X = Phi D for grad rho.  The unsymmetrised 2*128*K^2 figure is reported beside it.
+    f_rho = st["flops_rho_useful"] if gga else st["flops_rho_useful_sym"]
+    f_rho_exec = st["flops_rho_exec"] if gga else st["flops_rho_exec_sym"]
+    f_v = st["flops_v_useful"]
     f_total = f_rho + f_v
+    f_total_unsym = st["flops_rho_useful"] + f_v
     t_rho = stage_ms["rho"] * 1e-3
     roof = {"bound": "tensor", "kernel": "k_rho (rho contraction, DMMA.8x8x4)",
             "achieved": f_rho / t_rho / 1e12, "peak": fp64_clock_peak, "unit": "TFLOP/s",
@@ -266,10 +271,15 @@ def main():
                            f"MEASURED_PEAKS.json ({pk['_source']}); live DMMA microbenchmark "
                            f"{dmma_live and round(dmma_live, 2)} TFLOP/s; bf16-ratio rule would give "
                            f"{pk['bf16_tflops'] * 40.0 / 2250.0:.1f}",
-            "flops_per_launch": f_rho, "exec_flops_per_launch": st["flops_rho_exec"],
+            "flops_per_launch": f_rho, "exec_flops_per_launch": f_rho_exec,
+            "exec_frac": f_rho_exec / t_rho / 1e12 / fp64_clock_peak,
             "launch_ms": stage_ms["rho"], "traffic": None,
             "v_kernel": {"achieved": f_v / (stage_ms["vxc"] * 1e-3) / 1e12, "launch_ms": stage_ms["vxc"],
-                         "flops_per_launch": f_v, "exec_flops_per_launch": st["flops_v_exec"]}}
+                         "frac": f_v / (stage_ms["vxc"] * 1e-3) / 1e12 / fp64_clock_peak,
+                         "flops_per_launch": f_v, "exec_flops_per_launch": st["flops_v_exec"],
+                         "exec_frac": st["flops_v_exec"] / (stage_ms["vxc"] * 1e-3) / 1e12 / fp64_clock_peak,
+                         "schedule_critical_path_flops": st["flops_v_crit"],
+                         "deterministic": bool(args.deterministic_v)}}
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tr):
         try:
@@ -288,13 +298,15 @@ def main():
         "retained_block_tflops": f_total * world / (ms_per_step * 1e-3) / 1e12 if world == 1 else None,
         "retained_block_frac_of_fp64_peak": f_total / (ms_per_step * 1e-3) / 1e12 / fp64_clock_peak if world == 1 else None,
         "retained_block_frac_of_nominal_40tf": f_total / (ms_per_step * 1e-3) / 1e12 / 40.0 if world == 1 else None,
-        "flops": {"rho_useful": f_rho, "v_useful": f_v, "rho_exec": st["flops_rho_exec"], "v_exec": st["flops_v_exec"],
+        "retained_block_tflops_without_rho_symmetry": f_total_unsym / (ms_per_step * 1e-3) / 1e12 if world == 1 else None,
+        "flops": {"rho_useful": f_rho, "rho_useful_without_symmetry": st["flops_rho_useful"], "v_useful": f_v,
+                  "rho_exec": f_rho_exec, "v_exec": st["flops_v_exec"], "rho_symmetry_halving": not gga,
                   "dense_one_product": st["flops_dense"], "retained_over_dense": f_total / (2 * st["flops_dense"]),
                   "v_symmetry_halving": not gga, "ao_partition": "one AO block per shell"},
         "stage_ms": stage_ms, "plan_create_s": st["plan_seconds"], "workload_gen_s": gen_s, "exc_energy": E,
         "plan": {k: st[k] for k in ("n_blocks", "n_blocks_nonempty", "retained_blocks", "candidate_blocks", "sum_k",
                                      "max_k", "phi_bytes")},
-        "gpu_launches": 6 + (1 if gga else 0), "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+        "gpu_launches": 6 + (1 if gga else 0) + args.deterministic_v, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)
