@@ -280,13 +280,13 @@ def main():
                          "exec_frac": st["flops_v_exec"] / (stage_ms["vxc"] * 1e-3) / 1e12 / fp64_clock_peak,
                          "schedule_critical_path_flops": st["flops_v_crit"],
                          "deterministic": bool(args.deterministic_v)}}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")  # ncu --set full DRAM bytes per launch (text, committed)
     if os.path.exists(tr):
-        try:
-            with open(tr) as f:
-                roof["traffic"] = json.load(f).get(args.config, {}).get("k_rho_dram_bytes")
-        except Exception:
-            pass
+        with open(tr) as f:
+            for ln in f:
+                c = ln.strip().split(",")
+                if len(c) >= 3 and c[0] == args.config and c[1] == "k_rho" and abs(args.eps - 1e-12) < 1e-20:
+                    roof["traffic"] = int(c[2])
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
