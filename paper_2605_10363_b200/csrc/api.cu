@@ -105,10 +105,10 @@ kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells,
     const int k8 = (int)(P->h_panel_off[p + 1] - P->h_panel_off[p]);
     fr += 2.0 * GB * (double)k8 * k8;
     if (!k8) continue;
-    const int ntile = (k8 + 127) / 128, W = (((k8 + ntile - 1) / ntile) + 7) & ~7;
+    const int ntile = (k8 + 127) / 128, W = (((k8 + ntile - 1) / ntile) + 31) & ~31;
     for (int jt = 0; jt < ntile; ++jt) {
       const int n0 = jt * W, Wj = std::min(W, k8 - n0);
-      for (int k0 = (n0 / 32) * 32; k0 < k8; k0 += 32) {
+      for (int k0 = n0; k0 < k8; k0 += 32) {
         const int kc = std::min(32, k8 - k0);
         frs += 2.0 * GB * kc * (double)std::min(Wj, k0 + kc - n0);
       }

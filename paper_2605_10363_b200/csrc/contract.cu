@@ -65,6 +65,21 @@ __device__ __forceinline__ void rho_ksteps(double (&acc)[2][16][2], const double
   }
 }
 
+// TRI epilogue of the (up to 4) column groups J0.. that became final with this chunk: the Phi columns are the
+// chunk's own first columns in the stage.  es points at column 2 r4, row 16 warp + q4 of the stage.
+template <int J0>
+__device__ __forceinline__ void rho_epi_smem(const double (&acc)[2][16][2], double (&rs)[2],
+                                             const double* __restrict__ es, int ecnt) {
+#pragma unroll
+  for (int jj = 0; jj < 4; ++jj) {
+    if (jj < ecnt) {
+      const double* e = es + jj * 8 * LD;
+      rs[0] += acc[0][J0 + jj][0] * e[0] + acc[0][J0 + jj][1] * e[LD];
+      rs[1] += acc[1][J0 + jj][0] * e[8] + acc[1][J0 + jj][1] * e[LD + 8];
+    }
+  }
+}
+
 __device__ __forceinline__ void rho_stage(double (&acc)[2][16][2], const double* __restrict__ ps,
                                           const double* __restrict__ ds, int nks, int nj) {
   switch (nj) {
@@ -110,7 +125,8 @@ __global__ void __launch_bounds__(288, 1)
       const int K8 = (kp[p] + 7) & ~7;
       const int64_t base = panel_off[p];
       const int ntile = (K8 + NT - 1) / NT;
-      const int W = (((K8 + ntile - 1) / ntile) + 7) & ~7;
+      // TRI: tiles start on 32-column (K-chunk) boundaries so that a chunk's own columns are whole j-groups
+      const int W = TRI ? (((K8 + ntile - 1) / ntile) + 31) & ~31 : (((K8 + ntile - 1) / ntile) + 7) & ~7;
       for (int jt = 0; jt < ntile; ++jt) {
         const int n0 = jt * W, Wj = min(W, K8 - n0);
         int cn[4];
@@ -118,8 +134,13 @@ __global__ void __launch_bounds__(288, 1)
         for (int c = 0; c < 4; ++c) cn[c] = (lane + 32 * c < Wj) ? colidx[base + n0 + lane + 32 * c] : -1;
         // TRI: D' is lower triangular in packed order (colidx ascends), so chunk rows k < n0 contribute
         // nothing to this N-tile and a chunk [k0, k0+kc) only reaches the columns n < k0 + kc.
-        const int kstart = TRI ? (n0 / KC) * KC : 0;
-        for (int k0 = kstart; k0 < K8; k0 += KC) {
+        // TRI also walks the chunks in DESCENDING k: after chunk [k0, k0+kc) the columns n in that same range of
+        // X' = Phi D' are final (they only take k >= n) while their Phi columns are still in the stage, so the
+        // rho epilogue of those columns runs from shared memory, chunk by chunk, with no global re-read.
+        const int kstart = TRI ? n0 : 0;
+        const int nchunk = (K8 - kstart + KC - 1) / KC;
+        for (int ci = 0; ci < nchunk; ++ci) {
+          const int k0 = kstart + KC * (TRI ? nchunk - 1 - ci : ci);
           const int kc = min(KC, K8 - k0);
           const int wact = TRI ? min(Wj, k0 + kc - n0) : Wj;
           mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
@@ -127,15 +148,16 @@ __global__ void __launch_bounds__(288, 1)
           const uint32_t full = bar0 + 8 * s;
           if (lane == 0) {
             int fl = 0;
-            if (k0 == kstart) fl |= F_FIRST;
-            if (k0 + KC >= K8) {
+            if (ci == 0) fl |= F_FIRST;
+            if (ci == nchunk - 1) {
               fl |= F_LAST_TILE;
               if (jt == ntile - 1) fl |= F_LAST_PANEL;
             }
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = n0;
             hdr[4 * s + 2] = (kc >> 2) | ((wact >> 3) << 8) | (fl << 16);
-            hdr[4 * s + 3] = Wj >> 3;
+            const int ecnt = TRI ? max(0, min(kc, n0 + Wj - k0)) >> 3 : 0;  // final column groups of this chunk
+            hdr[4 * s + 3] = (Wj >> 3) | (((k0 - n0) >> 3) << 8) | (ecnt << 16);
             mbar_arrive_expect_tx(full, (uint32_t)kc * (GB * 8));
           }
           __syncwarp();
@@ -177,7 +199,7 @@ __global__ void __launch_bounds__(288, 1)
     const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
     const int fl = h2 >> 16;
     if (fl & F_DONE) break;
-    const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, nW = hdr[4 * s + 3];
+    const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, h3 = hdr[4 * s + 3], nW = h3 & 0xff;
     if (fl & F_FIRST) {
 #pragma unroll
       for (int j = 0; j < 16; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
@@ -185,6 +207,18 @@ __global__ void __launch_bounds__(288, 1)
     const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 16 * warp + q4;
     const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
     rho_stage(acc, ps, ds, nks, nj);
+    if (TRI) {
+      const int ecnt = h3 >> 16;
+      if (ecnt) {
+        const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 16 * warp + q4;
+        switch ((h3 >> 10) & 3) {  // first final column group / 4
+          case 0: rho_epi_smem<0>(acc, rs[0], es, ecnt); break;
+          case 1: rho_epi_smem<4>(acc, rs[0], es, ecnt); break;
+          case 2: rho_epi_smem<8>(acc, rs[0], es, ecnt); break;
+          default: rho_epi_smem<12>(acc, rs[0], es, ecnt); break;
+        }
+      }
+    }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
     if (++s == NST) { s = 0; ph ^= 1; }
@@ -194,7 +228,7 @@ __global__ void __launch_bounds__(288, 1)
       const int64_t off = (panel_off[p] + n0 + 2 * r4) * GB + 16 * warp + q4;
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
-        if (j < nW) {
+        if (!TRI && j < nW) {
           const int64_t o = off + (int64_t)j * 8 * GB;
           rs[0][0] += acc[0][j][0] * phi[o] + acc[0][j][1] * phi[o + GB];
           rs[0][1] += acc[1][j][0] * phi[o + 8] + acc[1][j][1] * phi[o + GB + 8];
