@@ -42,7 +42,9 @@ constexpr int NT = 128;                   // max N-tile width
 constexpr int PHI_BYTES = KC * LD * 8;    // 33,792
 constexpr int D_BYTES = KC * (NT + 4) * 8;  // 33,792
 constexpr int STAGE_BYTES = PHI_BYTES + D_BYTES;
-constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
+constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8 + 16;
+constexpr int NPW = 4;                    // producer warps: each stages 8 of the 32 chunk rows
+constexpr int NTHREADS = 32 * (8 + NPW);
 enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
 }  // namespace rho
 
@@ -92,7 +94,7 @@ __device__ __forceinline__ void rho_stage(double (&acc)[2][16][2], const double*
 }
 
 template <bool GGA, bool TRI>
-__global__ void __launch_bounds__(288, 1)
+__global__ void __launch_bounds__(rho::NTHREADS, 1)
     k_rho(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
           const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
@@ -105,21 +107,24 @@ __global__ void __launch_bounds__(288, 1)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) {
-      mbar_init(bar0 + 8 * s, 33);         // producer lane 0 (expect_tx) + 32 cp.async completions
+      mbar_init(bar0 + 8 * s, 1 + 32 * NPW);  // expect_tx arrive + one cp.async completion per producer lane
       mbar_init(bar0 + 8 * (NST + s), 8);  // one arrive per consumer warp
     }
     fence_mbar_init();
   }
   __syncthreads();
 
-  if (warp == 8) {
-    // ------------------------------------------------------------------ producer warp
+  if (warp >= 8) {
+    // ------------------------------------------------------------------ producer warps (in lockstep per task)
+    const int pw = warp - 8;
+    volatile int* task_slot = reinterpret_cast<volatile int*>(smem + NST * STAGE_BYTES + NST * 16 + 2 * NST * 8);
     int s = 0;
     uint32_t ph = 0;
     for (;;) {
-      int t = 0;
-      if (lane == 0) t = atomicAdd(ticket, 1);
-      t = __shfl_sync(0xffffffffu, t, 0);
+      if (pw == 0 && lane == 0) *task_slot = atomicAdd(ticket, 1);
+      asm volatile("bar.sync 1, %0;" ::"n"(32 * NPW) : "memory");
+      const int t = *task_slot;
+      asm volatile("bar.sync 1, %0;" ::"n"(32 * NPW) : "memory");
       if (t >= n_tasks) break;
       const int p = tasks[t];
       const int K8 = (kp[p] + 7) & ~7;
@@ -144,9 +149,10 @@ __global__ void __launch_bounds__(288, 1)
           const int kc = min(KC, K8 - k0);
           const int wact = TRI ? min(Wj, k0 + kc - n0) : Wj;
           mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
-          const int rowidx = (lane < kc) ? colidx[base + k0 + lane] : 0;
+          const int r0 = 8 * pw, r1 = min(kc, r0 + 8);  // this warp's rows of the chunk
+          const int rowidx = (r0 + lane < r1) ? colidx[base + k0 + r0 + lane] : 0;
           const uint32_t full = bar0 + 8 * s;
-          if (lane == 0) {
+          if (pw == 0 && lane == 0) {
             int fl = 0;
             if (ci == 0) fl |= F_FIRST;
             if (ci == nchunk - 1) {
@@ -163,9 +169,10 @@ __global__ void __launch_bounds__(288, 1)
           __syncwarp();
           const uint32_t sphi = smem_u32(smem + s * STAGE_BYTES);
           const uint32_t sd = sphi + PHI_BYTES;
-          if (lane < kc) bulk_g2s(sphi + lane * (LD * 8), phi + (base + k0 + lane) * GB, GB * 8, full);
-          for (int r = 0; r < kc; ++r) {
-            const int row = __shfl_sync(0xffffffffu, rowidx, r);
+          if (r0 + lane < r1)
+            bulk_g2s(sphi + (r0 + lane) * (LD * 8), phi + (base + k0 + r0 + lane) * GB, GB * 8, full);
+          for (int r = r0; r < r1; ++r) {
+            const int row = __shfl_sync(0xffffffffu, rowidx, r - r0);
             const double* drow = Dp + (int64_t)row * n_ao;
             const uint32_t dst = sd + (r * (NT + 4) + lane) * 8;
 #pragma unroll
@@ -178,7 +185,7 @@ __global__ void __launch_bounds__(288, 1)
       }
     }
     mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
-    if (lane == 0) {
+    if (pw == 0 && lane == 0) {
       hdr[4 * s + 2] = F_DONE << 16;
       mbar_arrive(bar0 + 8 * s);
     }
@@ -395,12 +402,12 @@ kldi_status launch_rho(kldi_plan* P, bool gga) {
   if (P->n_tasks == 0) return KLDI_OK;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   if (gga)
-    k_rho<true, false><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
+    k_rho<true, false><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
                                                            P->n_pad);
   else
-    k_rho<false, true><<<grid, 288, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
+    k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
                                                             nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad);
   KLDI_CUDA(cudaGetLastError());
