@@ -17,7 +17,8 @@ constexpr int RC = 32;              // grid rows (the MMA K dimension) per ring 
 constexpr int STR = RC;             // column stride in doubles: dense, the chunk swizzle of vlayout_off avoids conflicts
 constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row block of an odd last strip)
 constexpr int COLS_BYTES = NCOL * STR * 8;
-constexpr int STAGE_BYTES = COLS_BYTES + RC * 8;  // + wv chunk
+constexpr int IDX_OFF = COLS_BYTES + RC * 8;      // plan AO index of every staged column (for the epilogue)
+constexpr int STAGE_BYTES = IDX_OFF + ((NCOL * 4 + 127) / 128) * 128;  // columns + wv chunk + column indices
 constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
 enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
 }  // namespace vg
@@ -102,8 +103,9 @@ __global__ void __launch_bounds__(288, 1)
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = ps;
             hdr[4 * s + 2] = (rc == 0 ? F_FIRST : 0) | (rc == GB / RC - 1 ? F_LAST : 0);
-            hdr[4 * s + 3] = K8;
-            mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8)));
+            hdr[4 * s + 3] = K8 | (kp[p] << 16);
+            mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8) +
+                                                   ((ATOMIC && rc == GB / RC - 1) ? (P.c1_n + P.c2_n) * 4 : 0)));
           }
           __syncwarp();
           if (lane == 0) {  // one bulk copy per column interval: the slab is contiguous in the V layout
@@ -114,6 +116,10 @@ __global__ void __launch_bounds__(288, 1)
               bulk_g2s(sa + P.c1_n * (RC * 8), (GGA ? zmat : phi) + slab + (int64_t)P.c2_lo * RC,
                        (uint32_t)P.c2_n * (RC * 8), full);
             if (!GGA) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
+            if (ATOMIC && rc == GB / RC - 1) {  // last slab of the pass: column indices for the scatter epilogue
+              bulk_g2s(sa + IDX_OFF, colidx + base + P.c1_lo, (uint32_t)P.c1_n * 4, full);
+              if (P.c2_n) bulk_g2s(sa + IDX_OFF + P.c1_n * 4, colidx + base + P.c2_lo, (uint32_t)P.c2_n * 4, full);
+            }
           }
           if (++s == NST) { s = 0; ph ^= 1; }
         }
@@ -138,7 +144,8 @@ __global__ void __launch_bounds__(288, 1)
   uint32_t ph = 0;
   for (;;) {
     mbar_wait(bar0 + 8 * s, ph);
-    const int p = hdr[4 * s + 0], ps = hdr[4 * s + 1], fl = hdr[4 * s + 2], K8 = hdr[4 * s + 3];
+    const int p = hdr[4 * s + 0], ps = hdr[4 * s + 1], fl = hdr[4 * s + 2];
+    const int K8 = hdr[4 * s + 3] & 0xffff, K = hdr[4 * s + 3] >> 16;
     if (fl & F_DONE) break;
     if (fl & F_FIRST) {
       const VItem* it = items + ((int64_t)ps * V_WARPS + warp) * V_SLOTS;
@@ -165,13 +172,15 @@ __global__ void __launch_bounds__(288, 1)
         default: break;
       }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    const int* sidx = reinterpret_cast<const int*>(smem + s * STAGE_BYTES + IDX_OFF);
+    if (!(ATOMIC && (fl & F_LAST))) {  // the atomic epilogue still reads the stage's column indices
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    }
+    const int s_cur = s;
     if (++s == NST) { s = 0; ph ^= 1; }
 
     if (fl & F_LAST) {
-      const int K = kp[p];
-      const int64_t base = panel_off[p];
 #pragma unroll
       for (int k = 0; k < V_SLOTS; ++k) {
         const int nj = ia[k] >> 20;
@@ -182,14 +191,15 @@ __global__ void __launch_bounds__(288, 1)
           const int r = arow + 8 * mi + q4;
           if (ATOMIC) {
             if (r < K) {
-              const int64_t ci = (int64_t)colidx[base + r] * n_ao;
+              const int64_t ci = (int64_t)sidx[(ia[k] & 1023) + 8 * mi + q4] * n_ao;
+              const int* cidx = sidx + ((ia[k] >> 10) & 1023) + 2 * r4;
 #pragma unroll
               for (int j = 0; j < 4; ++j)
                 if (j < nj) {
 #pragma unroll
                   for (int e = 0; e < 2; ++e) {
                     const int c = bcol + 8 * j + 2 * r4 + e;
-                    if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + colidx[base + c], acc[k][mi][j][e]);
+                    if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + cidx[8 * j + e], acc[k][mi][j][e]);
                   }
                 }
             }
@@ -207,6 +217,10 @@ __global__ void __launch_bounds__(288, 1)
             }
           }
         }
+      }
+      if (ATOMIC) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s_cur));
       }
     }
   }
