@@ -18,7 +18,8 @@ constexpr int STR = RC;             // column stride in doubles: dense, the chun
 constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row block of an odd last strip)
 constexpr int COLS_BYTES = NCOL * STR * 8;
 constexpr int IDX_OFF = COLS_BYTES + RC * 8;      // plan AO index of every staged column (for the epilogue)
-constexpr int STAGE_BYTES = IDX_OFF + ((NCOL * 4 + 127) / 128) * 128;  // columns + wv chunk + column indices
+constexpr int ITEM_OFF = IDX_OFF + ((NCOL * 4 + 127) / 128) * 128;     // the pass's 32 VItems (first slab only)
+constexpr int STAGE_BYTES = ITEM_OFF + V_WARPS * V_SLOTS * 8;          // columns + wv chunk + column indices + items
 constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
 enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
 }  // namespace vg
@@ -105,7 +106,8 @@ __global__ void __launch_bounds__(288, 1)
             hdr[4 * s + 2] = (rc == 0 ? F_FIRST : 0) | (rc == GB / RC - 1 ? F_LAST : 0);
             hdr[4 * s + 3] = K8 | (kp[p] << 16);
             mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8) +
-                                                   ((ATOMIC && rc == GB / RC - 1) ? (P.c1_n + P.c2_n) * 4 : 0)));
+                                                   ((ATOMIC && rc == GB / RC - 1) ? (P.c1_n + P.c2_n) * 4 : 0) +
+                                                   (rc == 0 ? V_WARPS * V_SLOTS * 8 : 0)));
           }
           __syncwarp();
           if (lane == 0) {  // one bulk copy per column interval: the slab is contiguous in the V layout
@@ -116,6 +118,7 @@ __global__ void __launch_bounds__(288, 1)
               bulk_g2s(sa + P.c1_n * (RC * 8), (GGA ? zmat : phi) + slab + (int64_t)P.c2_lo * RC,
                        (uint32_t)P.c2_n * (RC * 8), full);
             if (!GGA) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
+            if (rc == 0) bulk_g2s(sa + ITEM_OFF, items + (int64_t)ps * V_WARPS * V_SLOTS, V_WARPS * V_SLOTS * 8, full);
             if (ATOMIC && rc == GB / RC - 1) {  // last slab of the pass: column indices for the scatter epilogue
               bulk_g2s(sa + IDX_OFF, colidx + base + P.c1_lo, (uint32_t)P.c1_n * 4, full);
               if (P.c2_n) bulk_g2s(sa + IDX_OFF + P.c1_n * 4, colidx + base + P.c2_lo, (uint32_t)P.c2_n * 4, full);
@@ -144,15 +147,15 @@ __global__ void __launch_bounds__(288, 1)
   uint32_t ph = 0;
   for (;;) {
     mbar_wait(bar0 + 8 * s, ph);
-    const int p = hdr[4 * s + 0], ps = hdr[4 * s + 1], fl = hdr[4 * s + 2];
+    const int p = hdr[4 * s + 0], fl = hdr[4 * s + 2];
     const int K8 = hdr[4 * s + 3] & 0xffff, K = hdr[4 * s + 3] >> 16;
     if (fl & F_DONE) break;
     if (fl & F_FIRST) {
-      const VItem* it = items + ((int64_t)ps * V_WARPS + warp) * V_SLOTS;
+      const VItem* it = reinterpret_cast<const VItem*>(smem + s * STAGE_BYTES + ITEM_OFF) + warp * V_SLOTS;
 #pragma unroll
       for (int k = 0; k < V_SLOTS; ++k) {
-        ia[k] = __ldg(&it[k].a);
-        ib[k] = __ldg(&it[k].b);
+        ia[k] = it[k].a;
+        ib[k] = it[k].b;
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[k][0][j][0] = acc[k][0][j][1] = acc[k][1][j][0] = acc[k][1][j][1] = 0.0;
       }
