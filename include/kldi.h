@@ -179,6 +179,17 @@ kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);
  * to [0, 2^20-1].  xyz, origin: HOST [3]. */
 uint64_t kldi_morton_key(const double* xyz, const double* origin);
 
+/* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
+ * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32
+ * {c1_lo, c1_n, c2_lo, c2_n, max_load, units, 0, 0}; items: [cap][32][2] int32 (8 warps x 4 slots:
+ * a = a_slot | b_slot << 10 | nj << 20, b = arow | bcol << 16).  *n_passes is always set; nothing is written
+ * if cap < *n_passes.  For tests of the host logic. */
+kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* items, int64_t cap, int64_t* n_passes);
+
+/* Host only: element offset (in doubles) of (column col, grid row row) of a K8-column panel that starts at packed
+ * column panel_off in the V layout (4 slabs of 32 rows, [col][32] each, 16-byte chunks XOR-swizzled by col & 7). */
+int64_t kldi_vlayout_offset(int64_t panel_off, int32_t K8, int32_t col, int32_t row);
+
 const char* kldi_last_error(void);
 
 #ifdef __cplusplus

@@ -21,7 +21,8 @@ KLDI_GGA_PBEX = 1
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
-    "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option",
+    "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
+    "kldi_vlayout_offset",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
 
@@ -85,8 +86,12 @@ def lib():
         L.kldi_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.kldi_morton_key.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.kldi_morton_key.restype = C.c_uint64
+        L.kldi_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.kldi_vsched_export.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
+        L.kldi_vlayout_offset.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
+        L.kldi_vlayout_offset.restype = C.c_int64
         for name in EXPORTED:
-            if name not in ("kldi_last_error", "kldi_morton_key"):
+            if name not in ("kldi_last_error", "kldi_morton_key", "kldi_vlayout_offset"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -241,6 +246,23 @@ def morton_key(xyz, origin) -> int:
     a = (C.c_double * 3)(*[float(v) for v in xyz])
     o = (C.c_double * 3)(*[float(v) for v in origin])
     return int(lib().kldi_morton_key(a, o))
+
+
+def vsched(nb: int, square: bool = False):
+    """Host-only: the V-contraction schedule of an nb-block panel -> (passes [n][8], items [n][32][2]) int32."""
+    import numpy as np
+
+    n = C.c_int64(0)
+    _check(lib().kldi_vsched_export(int(nb), int(square), None, None, 0, C.byref(n)), "kldi_vsched_export")
+    passes = np.zeros((n.value, 8), dtype=np.int32)
+    items = np.zeros((n.value, 32, 2), dtype=np.int32)
+    _check(lib().kldi_vsched_export(int(nb), int(square), passes.ctypes.data, items.ctypes.data, n.value,
+                                    C.byref(n)), "kldi_vsched_export")
+    return passes, items
+
+
+def vlayout_offset(panel_off: int, K8: int, col: int, row: int) -> int:
+    return int(lib().kldi_vlayout_offset(int(panel_off), int(K8), int(col), int(row)))
 
 
 def fp64_peak(kind: str = "dmma", iters: int = 20000) -> float:

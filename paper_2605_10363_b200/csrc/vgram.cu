@@ -5,6 +5,8 @@
 // device) and streams 32-row chunks of the panel columns a pass needs through a 3-stage mbarrier ring with
 // bulk-async copies (TMA engine, SASS UBLKCP); 8 consumer warps each hold up to 4 register-resident items
 // (16 rows x <= 32 columns) chosen by the host schedule of vsched.h, so that ragged K_p keeps every warp busy.
+#include <cstring>
+
 #include "kldi_internal.h"
 #include "ptx.cuh"
 #include "vsched.h"
@@ -447,3 +449,29 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
 }
 
 }  // namespace kldi
+
+extern "C" {
+
+kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* items, int64_t cap, int64_t* n_passes) {
+  if (nb < 0 || nb > 4095 || !n_passes) {
+    kldi::set_error("kldi_vsched_export: bad argument");
+    return KLDI_EINVAL;
+  }
+  std::vector<kldi::VPass> P;
+  std::vector<kldi::VItem> I;
+  if (nb > 0) kldi::vsched_build(nb, square != 0, P, I);
+  *n_passes = (int64_t)P.size();
+  if (!passes || !items || cap < *n_passes) return KLDI_OK;
+  static_assert(sizeof(kldi::VPass) == 32 && sizeof(kldi::VItem) == 8, "export layout");
+  if (!P.empty()) {
+    memcpy(passes, P.data(), P.size() * sizeof(kldi::VPass));
+    memcpy(items, I.data(), I.size() * sizeof(kldi::VItem));
+  }
+  return KLDI_OK;
+}
+
+int64_t kldi_vlayout_offset(int64_t panel_off, int32_t K8, int32_t col, int32_t row) {
+  return kldi::vlayout_off(panel_off, K8, col, row);
+}
+
+}  // extern "C"

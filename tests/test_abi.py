@@ -105,3 +105,75 @@ def test_morton_key_is_eq20(lib):
     assert binding.morton_key([-5.0, -5.0, -5.0], [0, 0, 0]) == 0              # below the origin -> 0
     # locality: points inside one 1/128-bohr cell share a key
     assert binding.morton_key([0.5001, 0.2501, 0.1251], [0, 0, 0]) == binding.morton_key([0.5003, 0.2503, 0.1253], [0, 0, 0])
+
+
+@pytest.mark.parametrize("square", [False, True])
+def test_v_schedule_covers_every_unit_once(square):
+    """Host logic of the V contraction (csrc/vsched.h): for every panel size the passes tile the (16-row strip,
+    8-column block) units of the Gram matrix exactly once (LDA: blocks on and above the strip's diagonal; GGA:
+    all), every item's operand columns lie inside the staged intervals, and no warp exceeds its 4 slots x 4
+    column blocks (64 FP64 accumulators per lane)."""
+    from paper_2605_10363_b200 import binding as K
+
+    for nb in list(range(1, 40)) + [47, 56, 64, 111]:
+        passes, items = K.vsched(nb, square)
+        ns = (nb + 1) // 2
+        seen = np.zeros((ns, nb), dtype=np.int32)
+        for P, I in zip(passes, items):
+            c1_lo, c1_n, c2_lo, c2_n, max_load, units = (int(v) for v in P[:6])
+            assert c1_n + c2_n <= 256 and c1_lo % 8 == 0 and c2_lo % 8 == 0 and c1_n % 8 == 0 and c2_n % 8 == 0
+            loads, tot = [], 0
+            for w in range(8):
+                load = 0
+                for k in range(4):
+                    a, b = int(I[w * 4 + k, 0]), int(I[w * 4 + k, 1])
+                    nj, a_slot, b_slot = a >> 20, a & 1023, (a >> 10) & 1023
+                    if nj == 0:
+                        continue
+                    assert 1 <= nj <= 4
+                    arow, bcol = b & 0xFFFF, b >> 16
+                    assert arow % 16 == 0 and bcol % 8 == 0
+                    # A rows come from interval 1; B columns from interval 1 (single interval) or interval 2
+                    assert c1_lo + a_slot == arow and a_slot + 8 <= c1_n + (8 if nb % 2 else 0) + 8
+                    if b_slot < c1_n and not square and c2_n == 0:
+                        assert c1_lo + b_slot == bcol and b_slot + 8 * nj <= c1_n
+                    else:
+                        assert b_slot >= c1_n and c2_lo + (b_slot - c1_n) == bcol and b_slot - c1_n + 8 * nj <= c2_n
+                    s = arow // 16
+                    for j in range(bcol // 8, bcol // 8 + nj):
+                        seen[s, j] += 1
+                    load += nj
+                loads.append(load)
+                tot += load
+            assert max(loads) == max_load <= 16 and tot == units
+        want = np.ones((ns, nb), dtype=np.int32)
+        if not square:
+            for s in range(ns):
+                want[s, : 2 * s] = 0
+        assert np.array_equal(seen, want), (nb, square)
+
+
+def test_v_layout_is_a_bijection_with_conflict_free_fragments():
+    """kldi_vlayout_offset: a permutation of the panel's elements; a slab's columns are contiguous; the 16-byte
+    chunks (2 r4 + j) of 8 adjacent columns fall into 8 different 16-byte bank groups for every quarter warp."""
+    from paper_2605_10363_b200 import binding as K
+
+    K8, po = 24, 40
+    offs = np.array([[K.vlayout_offset(po, K8, c, r) for r in range(128)] for c in range(K8)])
+    assert sorted(offs.ravel().tolist()) == list(range(po * 128, (po + K8) * 128))
+    for rc in range(4):
+        blk = offs[:, 32 * rc: 32 * rc + 32] - (po * 128 + rc * K8 * 32)
+        assert blk.min() == 0 and blk.max() == K8 * 32 - 1
+        for c in range(K8):
+            assert blk[c].min() == 32 * c and blk[c].max() == 32 * c + 31      # column c is one 256-byte run
+    for j in range(2):
+        for h in range(2):
+            for qpair in range(4):                                             # quarter warp: q4 in {2g, 2g+1}
+                groups = set()
+                for q4 in (2 * qpair, 2 * qpair + 1):
+                    for r4 in range(4):
+                        row = 2 * (2 * r4 + j + 8 * h)
+                        o = K.vlayout_offset(0, K8, 8 + q4, row)
+                        assert o % 2 == 0 and K.vlayout_offset(0, K8, 8 + q4, row + 1) == o + 1
+                        groups.add((o * 8 // 16) % 8)
+                assert len(groups) == 8
