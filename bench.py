@@ -153,6 +153,8 @@ def main():
     ap.add_argument("--eps", type=float, default=1e-12)
     ap.add_argument("--ref-sample", type=int, default=4096)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pair-test", type=int, default=0, choices=[0, 1],
+                    help="1: executable-pair selection a_pq*b_qr >= eps per call (Eq. 17-19)")
     ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1],
                     help="1: V without FP64 atomics (workspace partials + fixed-order reduce)")
     args = ap.parse_args()
@@ -193,6 +195,7 @@ def main():
     func = K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER
     plan = K.Plan.from_workload(wl)
     plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
+    plan.set_option(K.KLDI_OPT_PAIR_TEST, args.pair_test)
     st = plan.stats.as_dict()
     D = torch.as_tensor(wl.D, device="cuda")
     V = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")
@@ -306,7 +309,9 @@ def main():
         "stage_ms": stage_ms, "plan_create_s": st["plan_seconds"], "workload_gen_s": gen_s, "exc_energy": E,
         "plan": {k: st[k] for k in ("n_blocks", "n_blocks_nonempty", "retained_blocks", "candidate_blocks", "sum_k",
                                      "max_k", "phi_bytes")},
-        "gpu_launches": 6 + (1 if gga else 0) + args.deterministic_v, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+        "pair_test": {"enabled": bool(args.pair_test), "stages_total": plan.refresh_stats().pair_stages_total,
+                      "stages_executed": plan.stats.pair_stages_executed},
+        "gpu_launches": 6 + (1 if gga else 0) + args.deterministic_v + 2 * args.pair_test, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)

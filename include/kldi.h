@@ -99,6 +99,8 @@ typedef struct {
   double flops_rho_useful_sym; /* sum_p 128*K_p*(K_p+1): the LDA rho build, which uses D = D^T */
   double flops_rho_exec_sym;   /* FLOPs the LDA-form (triangular D) rho kernel issues */
   double flops_v_crit;         /* V kernel: 8 warps x the busiest warp's units, summed (schedule imbalance) */
+  int64_t pair_stages_total;   /* KLDI_OPT_PAIR_TEST, last rho call: (K chunk, N tile) stages before the test; -1 = off */
+  int64_t pair_stages_executed;/* ... and stages that contain an executable pair a_pq*b_qr >= eps (Eq. 17-19) */
 } kldi_stats;
 
 /* Once per geometry: Morton reorder of the grid into blocks of 128 (Eq. 20), spatial
@@ -163,11 +165,16 @@ kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_
 kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, double* out,
                                   int64_t cap_bytes, int32_t* width);
 
-/* Options of a plan.  KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram
- * tile into V with red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a
- * workspace (allocated on first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed
- * order: no FP64 atomics, V bitwise reproducible.  Returns KLDI_EINVAL for unknown options. */
-typedef enum { KLDI_OPT_DETERMINISTIC_V = 1 } kldi_option;
+/* Options of a plan (kldi_plan_set_option returns KLDI_EINVAL for an unknown option).
+ * KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram tile into V with
+ * red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a workspace (allocated on
+ * first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed order: no FP64 atomics, V bitwise
+ * reproducible.
+ * KLDI_OPT_PAIR_TEST: 0 (default) = the rho contraction executes every retained pair (E = I, the conservative
+ * superset); 1 = per call, b_qr = max|D_qr| is formed for every AO-shell pair and a (32-column K chunk, N tile)
+ * stage of the rho kernel runs only if it contains a pair with a_pq * b_qr >= eps (Eq. 17-19, t_d = eps); costs
+ * one pass over D and one over the retained-pair lists per call, pays off for a localised D. */
+typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2 } kldi_option;
 kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
 
 /* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`

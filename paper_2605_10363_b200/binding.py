@@ -25,6 +25,7 @@ EXPORTED = [
     "kldi_vlayout_offset",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
+KLDI_OPT_PAIR_TEST = 2
 
 
 class KldiError(RuntimeError):
@@ -53,6 +54,7 @@ class Stats(C.Structure):
         ("flops_rho_useful", C.c_double), ("flops_rho_exec", C.c_double), ("flops_v_useful", C.c_double),
         ("flops_v_exec", C.c_double), ("flops_dense", C.c_double), ("plan_seconds", C.c_double), ("eps", C.c_double),
         ("flops_rho_useful_sym", C.c_double), ("flops_rho_exec_sym", C.c_double), ("flops_v_crit", C.c_double),
+        ("pair_stages_total", C.c_int64), ("pair_stages_executed", C.c_int64),
     ]
 
     def as_dict(self) -> dict:
@@ -185,6 +187,13 @@ class Plan:
         _check(lib().kldi_build_vxc(self._h, self._dev64(wv, shape, "wv"), 1 if gga else 0,
                                     self._dev64(V, (self.n_ao, self.n_ao), "V")), "kldi_build_vxc")
         return V
+
+    def refresh_stats(self) -> "Stats":
+        """Re-reads kldi_plan_stats (the pair-test counters change per call)."""
+        st = Stats()
+        _check(lib().kldi_plan_stats(self._h, C.byref(st)), "kldi_plan_stats")
+        self.stats = st
+        return st
 
     def set_option(self, option: int, value: int):
         _check(lib().kldi_plan_set_option(self._h, int(option), int(value)), "kldi_plan_set_option")

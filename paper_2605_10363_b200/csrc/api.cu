@@ -133,6 +133,14 @@ kldi_status kldi_plan_stats(const kldi_plan* P, kldi_stats* out) {
     return KLDI_EINVAL;
   }
   *out = P->stats;
+  out->pair_stages_total = out->pair_stages_executed = -1;
+  if (P->pair_counts_valid) {  // counters of the most recent rho contraction run with KLDI_OPT_PAIR_TEST
+    unsigned long long c[2] = {0, 0};
+    KLDI_CUDA(cudaStreamSynchronize(P->stream));
+    KLDI_CUDA(cudaMemcpy(c, P->d_pcount, sizeof(c), cudaMemcpyDeviceToHost));
+    out->pair_stages_total = (int64_t)c[0];
+    out->pair_stages_executed = (int64_t)c[1];
+  }
   return KLDI_OK;
 }
 
@@ -246,11 +254,15 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
 }
 
 kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
-  if (!P || option != KLDI_OPT_DETERMINISTIC_V) {
+  if (!P || (option != KLDI_OPT_DETERMINISTIC_V && option != KLDI_OPT_PAIR_TEST)) {
     set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);
     return KLDI_EINVAL;
   }
-  P->v_mode = value ? 1 : 0;
+  if (option == KLDI_OPT_DETERMINISTIC_V) P->v_mode = value ? 1 : 0;
+  if (option == KLDI_OPT_PAIR_TEST) {
+    P->pair_test = value ? 1 : 0;
+    if (!value) P->pair_counts_valid = false;
+  }
   return KLDI_OK;
 }
 

@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
           const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
           const double* __restrict__ dphi2, const double* __restrict__ Dp, int n_ao, double* __restrict__ rho_s,
-          double* __restrict__ drho_s, int64_t n_pad) {
+          double* __restrict__ drho_s, int64_t n_pad, const unsigned long long* __restrict__ pmask) {
   using namespace rho;
   extern __shared__ __align__(128) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
@@ -130,6 +130,8 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
       const int K8 = (kp[p] + 7) & ~7;
       const int64_t base = panel_off[p];
       const int ntile = (K8 + NT - 1) / NT;
+      // executable-pair mask of this grid block (pairsel.cu; Eq. 19): bit (k0/32)*4 + jt, all ones = no test
+      const unsigned long long pm = pmask ? pmask[p] : ~0ull;
       // TRI: tiles start on 32-column (K-chunk) boundaries so that a chunk's own columns are whole j-groups
       const int W = TRI ? (((K8 + ntile - 1) / ntile) + 31) & ~31 : (((K8 + ntile - 1) / ntile) + 7) & ~7;
       for (int jt = 0; jt < ntile; ++jt) {
@@ -144,9 +146,15 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
         // rho epilogue of those columns runs from shared memory, chunk by chunk, with no global re-read.
         const int kstart = TRI ? n0 : 0;
         const int nchunk = (K8 - kstart + KC - 1) / KC;
+        bool started = false;
         for (int ci = 0; ci < nchunk; ++ci) {
           const int k0 = kstart + KC * (TRI ? nchunk - 1 - ci : ci);
           const int kc = min(KC, K8 - k0);
+          // a stage without an executable pair is skipped; the chunks that carry the tile's own columns (TRI:
+          // their epilogue runs in that stage) and the last stage of a tile (it closes the tile) always run
+          if (pm != ~0ull && !((pm >> (((k0 >> 5) & 15) * 4 + (jt & 3))) & 1ull) &&
+              (TRI ? k0 >= n0 + Wj : ci != nchunk - 1))
+            continue;
           const int wact = TRI ? min(Wj, k0 + kc - n0) : Wj;
           mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
           const int r0 = 8 * pw, r1 = min(kc, r0 + 8);  // this warp's rows of the chunk
@@ -154,7 +162,7 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
           const uint32_t full = bar0 + 8 * s;
           if (pw == 0 && lane == 0) {
             int fl = 0;
-            if (ci == 0) fl |= F_FIRST;
+            if (!started) fl |= F_FIRST;
             if (ci == nchunk - 1) {
               fl |= F_LAST_TILE;
               if (jt == ntile - 1) fl |= F_LAST_PANEL;
@@ -180,6 +188,7 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
               if (cn[c] >= 0 && lane + 32 * c < wact) cp_async8(dst + c * 256, drow + cn[c]);
           }
           cp_async_mbar_arrive_noinc(full);
+          started = true;
           if (++s == NST) { s = 0; ph ^= 1; }
         }
       }
@@ -400,16 +409,22 @@ kldi_status launch_rho(kldi_plan* P, bool gga) {
   if (gga) KLDI_CUDA(cudaMemsetAsync(P->d_drho_s, 0, sizeof(double) * 3 * P->n_pad, P->stream));
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
   if (P->n_tasks == 0) return KLDI_OK;
+  const unsigned long long* pm = nullptr;
+  if (P->pair_test) {
+    if ((rc = launch_pair_select(P, !gga)) != KLDI_OK) return rc;
+    pm = P->d_pmask;
+  }
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   if (gga)
     k_rho<true, false><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
-                                                           P->n_pad);
+                                                           P->n_pad, pm);
   else
     k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
-                                                            nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad);
+                                                            nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad,
+                                                            pm);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }

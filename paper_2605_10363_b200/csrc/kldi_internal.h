@@ -89,6 +89,12 @@ struct kldi_plan {
   int64_t gram_cap = 0;
   int32_t* d_ao_shell = nullptr;                  // plan AO -> plan shell
   int v_mode = 0;                                 // 0: red.global.add epilogue, 1: workspace + fixed-order reduce
+  // ---- executable-pair selection (pairsel.cu), allocated on first use
+  int pair_test = 0;
+  double* d_bmax = nullptr;                       // [n_shells][n_shells] b_qr = max|D_qr|
+  unsigned long long* d_pmask = nullptr;          // [n_blocks] stage masks, then 2 counters
+  unsigned long long* d_pcount = nullptr;         // -> d_pmask + n_blocks: {stages without the test, stages executed}
+  bool pair_counts_valid = false;
 
   // ---- task lists
   int32_t* d_tasks = nullptr;  // non-empty grid blocks in Morton order
@@ -116,6 +122,8 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
 void plan_free(kldi_plan* P);
 // contract.cu
 kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
+// pairsel.cu
+kldi_status launch_pair_select(kldi_plan* P, bool tri);
 kldi_status launch_rho(kldi_plan* P, bool gga);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);

@@ -323,6 +323,45 @@ def test_deterministic_v_mode(K, name, n, fn):
     plan.close()
 
 
+def _localised_D(wl, gamma):
+    """D o exp(-gamma R_AB^2): a symmetric density matrix that decays with the distance of the two AO centres."""
+    ncomp = {0: 1, 1: 3, 2: 6}
+    ao_atom = np.concatenate([np.full(ncomp[int(l)], int(a)) for a, l in zip(wl.shell_atom, wl.shell_l)])
+    xyz = np.asarray(wl.atom_xyz)[ao_atom]
+    r2 = ((xyz[:, None, :] - xyz[None, :, :]) ** 2).sum(-1)
+    return np.asarray(wl.D) * np.exp(-gamma * r2)
+
+
+@pytest.mark.parametrize("fn", ["lda", "gga"])
+def test_executable_pair_test(K, fn):
+    """KLDI_OPT_PAIR_TEST (Eq. 17-19): with a localised D whole (K chunk, N tile) stages hold no pair with
+    a_pq b_qr >= eps and are skipped; the result stays within the parity bar of the dense oracle on the same D,
+    and with the dense D of the configs (almost) every stage runs."""
+    import torch
+
+    wl = W.named_config("cfg1", n_override=16, functional=fn)
+    f = K.KLDI_GGA_PBEX if fn == "gga" else K.KLDI_LDA_SLATER
+    plan = K.Plan.from_workload(wl)
+    plan.set_option(K.KLDI_OPT_PAIR_TEST, 1)
+    for D, expect_skip in ((np.asarray(wl.D), False), (_localised_D(wl, 0.35), True)):
+        Dd = torch.as_tensor(D, device="cuda")
+        E, V = plan.exc(Dd, f)
+        st = plan.refresh_stats()
+        rho = plan.eval_rho(Dd)
+        ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, D, fn)
+        assert np.max(np.abs(rho.cpu().numpy() - ref["rho"])) <= TOL_RHO
+        assert np.max(np.abs(V.cpu().numpy() - ref["V"])) <= TOL_V
+        assert abs(E - ref["E"]) <= TOL_E
+        assert 0 < st.pair_stages_executed <= st.pair_stages_total
+        if expect_skip:
+            assert st.pair_stages_executed < st.pair_stages_total
+        else:  # dense D: (almost) every stage holds an executable pair
+            assert st.pair_stages_executed >= 0.98 * st.pair_stages_total
+    plan.set_option(K.KLDI_OPT_PAIR_TEST, 0)
+    assert plan.refresh_stats().pair_stages_total == -1
+    plan.close()
+
+
 @pytest.mark.parametrize("name", ["cfg3", "cfg4"])
 def test_full_size_sampled_parity(K, name):
     """BASELINE.json configs[3] / configs[4] at FULL size, in the launch configuration bench.py times:
