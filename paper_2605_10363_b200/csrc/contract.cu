@@ -45,7 +45,8 @@ constexpr int STAGE_BYTES = PHI_BYTES + D_BYTES;
 constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8 + 16;
 constexpr int NPW = 4;                    // producer warps: each stages 8 of the 32 chunk rows
 constexpr int NTHREADS = 32 * (8 + NPW);
-enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
+enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8, F_EPI = 16 };
+constexpr int EC = 16;                    // GGA epilogue stage: 16 tile columns of Phi, dxPhi, dyPhi, dzPhi
 }  // namespace rho
 
 // One ring stage of a consumer warp: nks k-steps of 4, NJ active 8-column groups (compile-time, so that no MMA
@@ -78,6 +79,24 @@ __device__ __forceinline__ void rho_epi_smem(const double (&acc)[2][16][2], doub
       const double* e = es + jj * 8 * LD;
       rs[0] += acc[0][J0 + jj][0] * e[0] + acc[0][J0 + jj][1] * e[LD];
       rs[1] += acc[1][J0 + jj][0] * e[8] + acc[1][J0 + jj][1] * e[LD + 8];
+    }
+  }
+}
+
+// GGA epilogue stage: column groups J0, J0+1 of the finished X tile against the staged Phi, dxPhi, dyPhi, dzPhi
+// columns ([array][16 columns][LD]); es points at column 2 r4, row 16 warp + q4 of array 0.
+template <int J0>
+__device__ __forceinline__ void rho_epi_gga(const double (&acc)[2][16][2], double (&rs)[4][2],
+                                            const double* __restrict__ es, int eb) {
+#pragma unroll
+  for (int jj = 0; jj < 2; ++jj) {
+    if (jj < eb) {
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        const double* e = es + (a * rho::EC + jj * 8) * LD;
+        rs[a][0] += acc[0][J0 + jj][0] * e[0] + acc[0][J0 + jj][1] * e[LD];
+        rs[a][1] += acc[1][J0 + jj][0] * e[8] + acc[1][J0 + jj][1] * e[LD + 8];
+      }
     }
   }
 }
@@ -164,8 +183,10 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
             int fl = 0;
             if (!started) fl |= F_FIRST;
             if (ci == nchunk - 1) {
-              fl |= F_LAST_TILE;
-              if (jt == ntile - 1) fl |= F_LAST_PANEL;
+              if (!GGA) {
+                fl |= F_LAST_TILE;
+                if (jt == ntile - 1) fl |= F_LAST_PANEL;
+              }
             }
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = n0;
@@ -190,6 +211,30 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
           cp_async_mbar_arrive_noinc(full);
           started = true;
           if (++s == NST) { s = 0; ph ^= 1; }
+        }
+        if (GGA) {
+          // epilogue operands through the ring: stage e holds columns [n0+16e, n0+16e+16) of the four stores,
+          // producer warp a stages array a; the consumers contract them with the finished X tile from shared memory
+          const double* arr = pw == 0 ? phi : pw == 1 ? dphi0 : pw == 2 ? dphi1 : dphi2;
+          const int nes = (Wj + EC - 1) / EC;
+          for (int e = 0; e < nes; ++e) {
+            const int ec = min(EC, Wj - EC * e);
+            mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
+            const uint32_t full = bar0 + 8 * s;
+            if (pw == 0 && lane == 0) {
+              hdr[4 * s + 0] = p;
+              hdr[4 * s + 1] = n0;
+              hdr[4 * s + 2] = (F_EPI | ((e == nes - 1 && jt == ntile - 1) ? F_LAST_PANEL : 0)) << 16;
+              hdr[4 * s + 3] = e | ((ec >> 3) << 8);
+              mbar_arrive_expect_tx(full, (uint32_t)(4 * ec) * (GB * 8));
+            }
+            __syncwarp();
+            if (lane < ec)
+              bulk_g2s(smem_u32(smem + s * STAGE_BYTES) + (pw * EC + lane) * (LD * 8),
+                       arr + (base + n0 + EC * e + lane) * GB, GB * 8, full);
+            cp_async_mbar_arrive_noinc(full);
+            if (++s == NST) { s = 0; ph ^= 1; }
+          }
         }
       }
     }
@@ -216,6 +261,18 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
     const int fl = h2 >> 16;
     if (fl & F_DONE) break;
     const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, h3 = hdr[4 * s + 3], nW = h3 & 0xff;
+    if (GGA && (fl & F_EPI)) {
+      if constexpr (GGA) {
+      const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 16 * warp + q4;
+      const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2)
+      switch (h3 & 0xff) {
+#define KLDI_CASE(E) case E: rho_epi_gga<2 * E>(acc, rs, es, eb); break;
+        KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7)
+#undef KLDI_CASE
+        default: break;
+      }
+      }
+    } else {
     if (fl & F_FIRST) {
 #pragma unroll
       for (int j = 0; j < 16; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
@@ -235,16 +292,17 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
         }
       }
     }
+    }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
     if (++s == NST) { s = 0; ph ^= 1; }
 
-    if (fl & F_LAST_TILE) {
+    if (fl & (F_LAST_TILE | F_LAST_PANEL)) {
       // epilogue: rho_p += rowsum(Phi_p[:, tile] o X[:, tile]); GGA: d_c rho_p += 2 rowsum(d_c Phi o X)
       const int64_t off = (panel_off[p] + n0 + 2 * r4) * GB + 16 * warp + q4;
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
-        if (!TRI && j < nW) {
+        if (!TRI && !GGA && j < nW) {
           const int64_t o = off + (int64_t)j * 8 * GB;
           rs[0][0] += acc[0][j][0] * phi[o] + acc[0][j][1] * phi[o + GB];
           rs[0][1] += acc[1][j][0] * phi[o + 8] + acc[1][j][1] * phi[o + GB + 8];
