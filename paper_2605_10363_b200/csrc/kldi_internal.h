@@ -18,9 +18,10 @@ void set_error(const char* fmt, ...);
 // rc holds [K8 columns][32 rows] contiguously, so any column interval of a slab is ONE bulk copy; inside a
 // column the 16-byte chunk c (rows 2c, 2c+1) sits at chunk c ^ (col & 7), which makes the 16-byte MMA
 // fragment loads of 8 adjacent columns bank-conflict free without padding (the smem image is the HBM image).
+constexpr int V_SLAB = 32;  // grid rows per slab of the V layout = MMA K rows per ring stage of k_vgram
 __host__ __device__ __forceinline__ int64_t vlayout_off(int64_t panel_off_p, int K8, int col, int row) {
-  const int rc = row >> 5, rr = row & 31, c = rr >> 1;
-  return panel_off_p * GB + (int64_t)rc * K8 * 32 + (int64_t)col * 32 + (((c ^ (col & 7)) << 1) | (rr & 1));
+  const int rc = row / V_SLAB, rr = row % V_SLAB, c = rr >> 1;
+  return panel_off_p * GB + (int64_t)rc * K8 * V_SLAB + (int64_t)col * V_SLAB + (((c ^ (col & 7)) << 1) | (rr & 1));
 }
 
 #define KLDI_CUDA(call)                                                                     \

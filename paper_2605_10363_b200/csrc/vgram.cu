@@ -14,8 +14,8 @@
 namespace kldi {
 
 namespace vg {
-constexpr int NST = 3;
-constexpr int RC = 32;              // grid rows (the MMA K dimension) per ring stage = one slab of the V layout
+constexpr int NST = V_SLAB == 16 ? 6 : 3;
+constexpr int RC = V_SLAB;              // grid rows (the MMA K dimension) per ring stage = one slab of the V layout
 constexpr int STR = RC;             // column stride in doubles: dense, the chunk swizzle of vlayout_off avoids conflicts
 constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row block of an odd last strip)
 constexpr int COLS_BYTES = NCOL * STR * 8;
@@ -33,7 +33,7 @@ __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __r
                                        const double* __restrict__ B, const double* __restrict__ w, int o0, int o1) {
   using namespace vg;
 #pragma unroll
-  for (int h = 0; h < 2; ++h) {
+  for (int h = 0; h < RC / 16; ++h) {
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
       const int o = (j ? o1 : o0) + 16 * h;
