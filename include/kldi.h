@@ -188,8 +188,8 @@ uint64_t kldi_morton_key(const double* xyz, const double* origin);
 
 /* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
  * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32
- * {c1_lo, c1_n, c2_lo, c2_n, max_load, units, 0, 0}; items: [cap][32][2] int32 (8 warps x 4 slots:
- * a = a_slot | b_slot << 10 | nj << 20, b = arow | bcol << 16).  *n_passes is always set; nothing is written
+ * {c1_lo, c1_n, c2_lo, c2_n, max_load, units, n_warps, n_slots}; items: [cap][32][2] int32 (item
+ * warp * n_slots + slot of the pass, the rest zero: a = a_slot | b_slot << 10 | nj << 20, b = arow | bcol << 16).  *n_passes is always set; nothing is written
  * if cap < *n_passes.  For tests of the host logic. */
 kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* items, int64_t cap, int64_t* n_passes);
 

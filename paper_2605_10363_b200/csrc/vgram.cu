@@ -3,8 +3,9 @@
 // (DMMA.8x8x4) and added to V (Eq. 5/16; accumulate-before-write-back).
 // Persistent, warp-specialised: a producer warp pulls grid blocks from an atomic ticket (on
 // device) and streams 32-row chunks of the panel columns a pass needs through a 3-stage mbarrier ring with
-// bulk-async copies (TMA engine, SASS UBLKCP); 8 consumer warps each hold up to 4 register-resident items
-// (16 rows x <= 32 columns) chosen by the host schedule of vsched.h, so that ragged K_p keeps every warp busy.
+// bulk-async copies (TMA engine, SASS UBLKCP); V_WARPS (15) consumer warps each hold up to V_SLOTS (2)
+// register-resident items (16 rows x <= 32 columns) chosen by the host schedule of vsched.h, so that ragged K_p
+// keeps every warp busy.
 #include <cstring>
 
 #include "kldi_internal.h"
@@ -21,7 +22,7 @@ constexpr int NCOL = V_MAXCOLS + 8; // column slots per stage (+8: second row bl
 constexpr int COLS_BYTES = NCOL * STR * 8;
 constexpr int IDX_OFF = COLS_BYTES + RC * 8;      // plan AO index of every staged column (for the epilogue)
 constexpr int ITEM_OFF = IDX_OFF + ((NCOL * 4 + 127) / 128) * 128;     // the pass's 32 VItems (first slab only)
-constexpr int STAGE_BYTES = ITEM_OFF + V_WARPS * V_SLOTS * 8;          // columns + wv chunk + column indices + items
+constexpr int STAGE_BYTES = ITEM_OFF + ((V_ITEMS * 8 + 127) / 128) * 128;          // columns + wv chunk + column indices + items
 constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8;
 enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
 }  // namespace vg
@@ -64,7 +65,7 @@ __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __r
 // ATOMIC = true : the epilogue adds G_p straight into the plan-order V with red.global.add.f64.
 // ATOMIC = false: G_p goes to the workspace (plain 16-B stores) and k_vreduce sums it in a fixed order.
 template <bool GGA, bool ATOMIC>
-__global__ void __launch_bounds__(288, 1)
+__global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
     k_vgram(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
             const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
             const double* __restrict__ phi, const double* __restrict__ zmat, const double* __restrict__ wv_s,
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(288, 1)
             hdr[4 * s + 3] = K8 | (kp[p] << 16);
             mbar_arrive_expect_tx(full, (uint32_t)((P.c1_n + P.c2_n) * (RC * 8) + (GGA ? 0 : RC * 8) +
                                                    ((ATOMIC && rc == GB / RC - 1) ? (P.c1_n + P.c2_n) * 4 : 0) +
-                                                   (rc == 0 ? V_WARPS * V_SLOTS * 8 : 0)));
+                                                   (rc == 0 ? V_ITEMS * 8 : 0)));
           }
           __syncwarp();
           if (lane == 0) {  // one bulk copy per column interval: the slab is contiguous in the V layout
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(288, 1)
               bulk_g2s(sa + P.c1_n * (RC * 8), (GGA ? zmat : phi) + slab + (int64_t)P.c2_lo * RC,
                        (uint32_t)P.c2_n * (RC * 8), full);
             if (!GGA) bulk_g2s(sa + COLS_BYTES, wv_s + (int64_t)p * GB + rc * RC, RC * 8, full);
-            if (rc == 0) bulk_g2s(sa + ITEM_OFF, items + (int64_t)ps * V_WARPS * V_SLOTS, V_WARPS * V_SLOTS * 8, full);
+            if (rc == 0) bulk_g2s(sa + ITEM_OFF, items + (int64_t)ps * V_ITEMS, V_ITEMS * 8, full);
             if (ATOMIC && rc == GB / RC - 1) {  // last slab of the pass: column indices for the scatter epilogue
               bulk_g2s(sa + IDX_OFF, colidx + base + P.c1_lo, (uint32_t)P.c1_n * 4, full);
               if (P.c2_n) bulk_g2s(sa + IDX_OFF + P.c1_n * 4, colidx + base + P.c2_lo, (uint32_t)P.c2_n * 4, full);
@@ -463,9 +464,14 @@ kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* ite
   *n_passes = (int64_t)P.size();
   if (!passes || !items || cap < *n_passes) return KLDI_OK;
   static_assert(sizeof(kldi::VPass) == 32 && sizeof(kldi::VItem) == 8, "export layout");
-  if (!P.empty()) {
-    memcpy(passes, P.data(), P.size() * sizeof(kldi::VPass));
-    memcpy(items, I.data(), I.size() * sizeof(kldi::VItem));
+  static_assert(kldi::V_ITEMS <= 32, "kldi_vsched_export documents 32 item slots per pass");
+  memset(items, 0, (size_t)*n_passes * 32 * sizeof(kldi::VItem));
+  for (size_t i = 0; i < P.size(); ++i) {
+    kldi::VPass q = P[i];
+    q.pad0 = kldi::V_WARPS;  // shape of the schedule, for the caller
+    q.pad1 = kldi::V_SLOTS;
+    memcpy(passes + 8 * i, &q, sizeof(q));
+    memcpy(items + 64 * i, I.data() + i * kldi::V_ITEMS, kldi::V_ITEMS * sizeof(kldi::VItem));
   }
   return KLDI_OK;
 }

@@ -1,8 +1,10 @@
 // Host-side schedule of the V (Gram) contraction for one grid block whose packed panel has nb column
 // blocks of 8 (K8 = 8 nb).  The output G = Phi^T diag(wv) Phi (LDA: upper triangle in 16-row strips;
 // GGA: the full square B = Phi^T Z) is cut into passes; a pass is a band of <= 8 strips x a range of
-// column blocks whose accumulators fit the registers of 8 consumer warps (4 slots of <= 4 column blocks
-// per warp = 64 FP64 accumulators per lane) and whose operand columns fit one ring stage (<= 256).
+// column blocks whose accumulators fit the registers of V_WARPS consumer warps (V_SLOTS slots of <= V_PIECE
+// column blocks per warp: 15 x 2 x 4 -> 32 FP64 accumulators per lane, 128 registers per thread, 16 warps per SM;
+// measured on cfg3: 8x4 5.46 ms, 11x3 4.70, 11x4 5.20, 15x3 5.06, 15x2 4.48) and whose operand columns fit one
+// ring stage (<= 256).
 // Inside a pass the strips are cut into pieces of <= 4 column blocks and spread over the warps by
 // longest-processing-time-first, so that ragged K_p does not leave warps idle.  This is the on-device
 // counterpart of the paper's pair selection + dense multiplier split.
@@ -14,7 +16,8 @@
 
 namespace kldi {
 
-constexpr int V_WARPS = 8, V_SLOTS = 4, V_PIECE = 4, V_BAND = 8, V_MAXCOLS = 256;
+constexpr int V_WARPS = 15, V_SLOTS = 2, V_PIECE = 4, V_BAND = 8, V_MAXCOLS = 256;
+constexpr int V_ITEMS = (V_WARPS * V_SLOTS + 1) & ~1;  // VItems stored per pass (even: 16-byte bulk copies)
 
 struct VItem {      // one slot of one consumer warp in one pass
   int32_t a;        // a_slot | b_slot << 10 | nj << 20   (stage-buffer column slots, nj = column blocks)
@@ -69,7 +72,7 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
       // pieces: try piece widths 4..1 and keep the assignment with the smallest maximum warp load
       struct Piece { int s, j0, nj; };
       const size_t item0 = items.size();
-      items.resize(item0 + V_WARPS * V_SLOTS, VItem{0, 0});
+      items.resize(item0 + V_ITEMS, VItem{0, 0});
       int best_load = 1 << 30;
       for (int pw = V_PIECE; pw >= 1; --pw) {
         std::vector<Piece> pc;

@@ -111,8 +111,8 @@ def test_morton_key_is_eq20(lib):
 def test_v_schedule_covers_every_unit_once(square):
     """Host logic of the V contraction (csrc/vsched.h): for every panel size the passes tile the (16-row strip,
     8-column block) units of the Gram matrix exactly once (LDA: blocks on and above the strip's diagonal; GGA:
-    all), every item's operand columns lie inside the staged intervals, and no warp exceeds its 4 slots x 4
-    column blocks (64 FP64 accumulators per lane)."""
+    all), every item's operand columns lie inside the staged intervals, and no warp exceeds its slots x 4
+    column blocks (its register-resident accumulators)."""
     from paper_2605_10363_b200 import binding as K
 
     for nb in list(range(1, 40)) + [47, 56, 64, 111]:
@@ -120,13 +120,14 @@ def test_v_schedule_covers_every_unit_once(square):
         ns = (nb + 1) // 2
         seen = np.zeros((ns, nb), dtype=np.int32)
         for P, I in zip(passes, items):
-            c1_lo, c1_n, c2_lo, c2_n, max_load, units = (int(v) for v in P[:6])
+            c1_lo, c1_n, c2_lo, c2_n, max_load, units, n_warps, n_slots = (int(v) for v in P[:8])
+            assert n_warps * n_slots <= 32
             assert c1_n + c2_n <= 256 and c1_lo % 8 == 0 and c2_lo % 8 == 0 and c1_n % 8 == 0 and c2_n % 8 == 0
             loads, tot = [], 0
-            for w in range(8):
+            for w in range(n_warps):
                 load = 0
-                for k in range(4):
-                    a, b = int(I[w * 4 + k, 0]), int(I[w * 4 + k, 1])
+                for k in range(n_slots):
+                    a, b = int(I[w * n_slots + k, 0]), int(I[w * n_slots + k, 1])
                     nj, a_slot, b_slot = a >> 20, a & 1023, (a >> 10) & 1023
                     if nj == 0:
                         continue
@@ -145,7 +146,7 @@ def test_v_schedule_covers_every_unit_once(square):
                     load += nj
                 loads.append(load)
                 tot += load
-            assert max(loads) == max_load <= 16 and tot == units
+            assert max(loads) == max_load <= 4 * n_slots and tot == units
         want = np.ones((ns, nb), dtype=np.int32)
         if not square:
             for s in range(ns):
