@@ -43,65 +43,67 @@ constexpr int PHI_BYTES = KC * LD * 8;    // 33,792
 constexpr int D_BYTES = KC * (NT + 4) * 8;  // 33,792
 constexpr int STAGE_BYTES = PHI_BYTES + D_BYTES;
 constexpr int SMEM_BYTES = NST * STAGE_BYTES + NST * 16 + 2 * NST * 8 + 16;
+constexpr int NCW = 16;                   // consumer warps: 8 grid rows each, all N columns
 constexpr int NPW = 4;                    // producer warps: each stages 8 of the 32 chunk rows
-constexpr int NTHREADS = 32 * (8 + NPW);
+constexpr int NTHREADS = 32 * (NCW + NPW);
 enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8, F_EPI = 16 };
 constexpr int EC = 16;                    // GGA epilogue stage: 16 tile columns of Phi, dxPhi, dyPhi, dzPhi
 }  // namespace rho
 
-// One ring stage of a consumer warp: nks k-steps of 4, NJ active 8-column groups (compile-time, so that no MMA
-// is predicated: a predicated mma.sync costs a WARPSYNC + NOP pair around every DMMA).
+// One ring stage of a consumer warp (8 grid rows x all N columns): nks k-steps of 4, NJ active 8-column groups
+// (compile-time, so that no MMA is predicated: a predicated mma.sync costs a WARPSYNC + NOP pair around every
+// DMMA).  B fragments are loaded 8 at a time to stay inside the 96-register budget of 20 warps per SM.
 template <int NJ>
-__device__ __forceinline__ void rho_ksteps(double (&acc)[2][16][2], const double* __restrict__ ps,
+__device__ __forceinline__ void rho_ksteps(double (&acc)[16][2], const double* __restrict__ ps,
                                            const double* __restrict__ ds, int nks) {
 #pragma unroll 2
   for (int ks = 0; ks < nks; ++ks) {
-    const double a0 = ps[ks * 4 * LD], a1 = ps[ks * 4 * LD + 8];
-    double b[NJ];
+    const double a = ps[ks * 4 * LD];
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) b[j] = ds[ks * 4 * (rho::NT + 4) + 8 * j];
+    for (int j0 = 0; j0 < NJ; j0 += 8) {
+      double b[8];
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-      dmma884(acc[0][j][0], acc[0][j][1], a0, b[j]);
-      dmma884(acc[1][j][0], acc[1][j][1], a1, b[j]);
+      for (int j = 0; j < 8; ++j)
+        if (j0 + j < NJ) b[j] = ds[ks * 4 * (rho::NT + 4) + 8 * (j0 + j)];
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if (j0 + j < NJ) dmma884(acc[j0 + j][0], acc[j0 + j][1], a, b[j]);
     }
   }
 }
 
 // TRI epilogue of the (up to 4) column groups J0.. that became final with this chunk: the Phi columns are the
-// chunk's own first columns in the stage.  es points at column 2 r4, row 16 warp + q4 of the stage.
+// chunk's own first columns in the stage.  es points at column 2 r4, row 8 warp + q4 of the stage.
 template <int J0>
-__device__ __forceinline__ void rho_epi_smem(const double (&acc)[2][16][2], double (&rs)[2],
-                                             const double* __restrict__ es, int ecnt) {
+__device__ __forceinline__ void rho_epi_smem(const double (&acc)[16][2], double& rs, const double* __restrict__ es,
+                                             int ecnt) {
 #pragma unroll
   for (int jj = 0; jj < 4; ++jj) {
     if (jj < ecnt) {
       const double* e = es + jj * 8 * LD;
-      rs[0] += acc[0][J0 + jj][0] * e[0] + acc[0][J0 + jj][1] * e[LD];
-      rs[1] += acc[1][J0 + jj][0] * e[8] + acc[1][J0 + jj][1] * e[LD + 8];
+      rs += acc[J0 + jj][0] * e[0] + acc[J0 + jj][1] * e[LD];
     }
   }
 }
 
 // GGA epilogue stage: column groups J0, J0+1 of the finished X tile against the staged Phi, dxPhi, dyPhi, dzPhi
-// columns ([array][16 columns][LD]); es points at column 2 r4, row 16 warp + q4 of array 0.
+// columns ([array][16 columns][LD]); es points at column 2 r4, row 8 warp + q4 of array 0.
 template <int J0>
-__device__ __forceinline__ void rho_epi_gga(const double (&acc)[2][16][2], double (&rs)[4][2],
-                                            const double* __restrict__ es, int eb) {
+__device__ __forceinline__ void rho_epi_gga(const double (&acc)[16][2], double (&rs)[4], const double* __restrict__ es,
+                                            int eb) {
 #pragma unroll
   for (int jj = 0; jj < 2; ++jj) {
     if (jj < eb) {
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
         const double* e = es + (a * rho::EC + jj * 8) * LD;
-        rs[a][0] += acc[0][J0 + jj][0] * e[0] + acc[0][J0 + jj][1] * e[LD];
-        rs[a][1] += acc[1][J0 + jj][0] * e[8] + acc[1][J0 + jj][1] * e[LD + 8];
+        rs[a] += acc[J0 + jj][0] * e[0] + acc[J0 + jj][1] * e[LD];
       }
     }
   }
 }
 
-__device__ __forceinline__ void rho_stage(double (&acc)[2][16][2], const double* __restrict__ ps,
+__device__ __forceinline__ void rho_stage(double (&acc)[16][2], const double* __restrict__ ps,
                                           const double* __restrict__ ds, int nks, int nj) {
   switch (nj) {
 #define KLDI_CASE(N) case N: rho_ksteps<N>(acc, ps, ds, nks); break;
@@ -127,15 +129,15 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) {
       mbar_init(bar0 + 8 * s, 1 + 32 * NPW);  // expect_tx arrive + one cp.async completion per producer lane
-      mbar_init(bar0 + 8 * (NST + s), 8);  // one arrive per consumer warp
+      mbar_init(bar0 + 8 * (NST + s), NCW);  // one arrive per consumer warp
     }
     fence_mbar_init();
   }
   __syncthreads();
 
-  if (warp >= 8) {
+  if (warp >= NCW) {
     // ------------------------------------------------------------------ producer warps (in lockstep per task)
-    const int pw = warp - 8;
+    const int pw = warp - NCW;
     volatile int* task_slot = reinterpret_cast<volatile int*>(smem + NST * STAGE_BYTES + NST * 16 + 2 * NST * 8);
     int s = 0;
     uint32_t ph = 0;
@@ -247,92 +249,69 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
     return;
   }
 
-  // -------------------------------------------------------------------- consumer warps (16 rows each)
-  double acc[2][16][2];
-  double rs[GGA ? 4 : 1][2];
+  // -------------------------------------------------------------------- consumer warps (8 rows each)
+  double acc[16][2];
+  double rs[GGA ? 4 : 1];
 #pragma unroll
-  for (int c = 0; c < (GGA ? 4 : 1); ++c) rs[c][0] = rs[c][1] = 0.0;
+  for (int c = 0; c < (GGA ? 4 : 1); ++c) rs[c] = 0.0;
   int s = 0;
   uint32_t ph = 0;
   const int q4 = lane >> 2, r4 = lane & 3;
   for (;;) {
     mbar_wait(bar0 + 8 * s, ph);
-    const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1], h2 = hdr[4 * s + 2];
+    const int p = hdr[4 * s + 0], h2 = hdr[4 * s + 2];
     const int fl = h2 >> 16;
     if (fl & F_DONE) break;
-    const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, h3 = hdr[4 * s + 3], nW = h3 & 0xff;
+    const int nks = h2 & 0xff, nj = (h2 >> 8) & 0xff, h3 = hdr[4 * s + 3];
+    const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 8 * warp + q4;
     if (GGA && (fl & F_EPI)) {
       if constexpr (GGA) {
-      const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 16 * warp + q4;
-      const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2)
-      switch (h3 & 0xff) {
+        const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2)
+        switch (h3 & 0xff) {
 #define KLDI_CASE(E) case E: rho_epi_gga<2 * E>(acc, rs, es, eb); break;
-        KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7)
+          KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7)
 #undef KLDI_CASE
-        default: break;
-      }
-      }
-    } else {
-    if (fl & F_FIRST) {
-#pragma unroll
-      for (int j = 0; j < 16; ++j) acc[0][j][0] = acc[0][j][1] = acc[1][j][0] = acc[1][j][1] = 0.0;
-    }
-    const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 16 * warp + q4;
-    const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
-    rho_stage(acc, ps, ds, nks, nj);
-    if (TRI) {
-      const int ecnt = h3 >> 16;
-      if (ecnt) {
-        const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 16 * warp + q4;
-        switch ((h3 >> 10) & 3) {  // first final column group / 4
-          case 0: rho_epi_smem<0>(acc, rs[0], es, ecnt); break;
-          case 1: rho_epi_smem<4>(acc, rs[0], es, ecnt); break;
-          case 2: rho_epi_smem<8>(acc, rs[0], es, ecnt); break;
-          default: rho_epi_smem<12>(acc, rs[0], es, ecnt); break;
+          default: break;
         }
       }
-    }
+    } else {
+      if (fl & F_FIRST) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) acc[j][0] = acc[j][1] = 0.0;
+      }
+      const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 8 * warp + q4;
+      const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
+      rho_stage(acc, ps, ds, nks, nj);
+      if (TRI) {
+        const int ecnt = h3 >> 16;
+        if (ecnt) {
+          switch ((h3 >> 10) & 3) {  // first final column group / 4
+            case 0: rho_epi_smem<0>(acc, rs[0], es, ecnt); break;
+            case 1: rho_epi_smem<4>(acc, rs[0], es, ecnt); break;
+            case 2: rho_epi_smem<8>(acc, rs[0], es, ecnt); break;
+            default: rho_epi_smem<12>(acc, rs[0], es, ecnt); break;
+          }
+        }
+      }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
     if (++s == NST) { s = 0; ph ^= 1; }
 
-    if (fl & (F_LAST_TILE | F_LAST_PANEL)) {
-      // epilogue: rho_p += rowsum(Phi_p[:, tile] o X[:, tile]); GGA: d_c rho_p += 2 rowsum(d_c Phi o X)
-      const int64_t off = (panel_off[p] + n0 + 2 * r4) * GB + 16 * warp + q4;
+    if (fl & F_LAST_PANEL) {  // rho_p (and grad rho_p) of this warp's 8 rows: quad reduction, one store per row
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        if (!TRI && !GGA && j < nW) {
-          const int64_t o = off + (int64_t)j * 8 * GB;
-          rs[0][0] += acc[0][j][0] * phi[o] + acc[0][j][1] * phi[o + GB];
-          rs[0][1] += acc[1][j][0] * phi[o + 8] + acc[1][j][1] * phi[o + GB + 8];
-          if (GGA) {
-            rs[1][0] += acc[0][j][0] * dphi0[o] + acc[0][j][1] * dphi0[o + GB];
-            rs[1][1] += acc[1][j][0] * dphi0[o + 8] + acc[1][j][1] * dphi0[o + GB + 8];
-            rs[2][0] += acc[0][j][0] * dphi1[o] + acc[0][j][1] * dphi1[o + GB];
-            rs[2][1] += acc[1][j][0] * dphi1[o + 8] + acc[1][j][1] * dphi1[o + GB + 8];
-            rs[3][0] += acc[0][j][0] * dphi2[o] + acc[0][j][1] * dphi2[o + GB];
-            rs[3][1] += acc[1][j][0] * dphi2[o + 8] + acc[1][j][1] * dphi2[o + GB + 8];
-          }
+      for (int c = 0; c < (GGA ? 4 : 1); ++c) {
+        double v = rs[c];
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        if (r4 == 0) {
+          const int64_t g = (int64_t)p * GB + 8 * warp + q4;
+          if (c == 0)
+            rho_s[g] = TRI ? 2.0 * v : v;
+          else
+            drho_s[(int64_t)(c - 1) * n_pad + g] = 2.0 * v;
         }
-      }
-      if (fl & F_LAST_PANEL) {
-#pragma unroll
-        for (int c = 0; c < (GGA ? 4 : 1); ++c)
-#pragma unroll
-          for (int mi = 0; mi < 2; ++mi) {
-            double v = rs[c][mi];
-            v += __shfl_xor_sync(0xffffffffu, v, 1);
-            v += __shfl_xor_sync(0xffffffffu, v, 2);
-            if (r4 == 0) {
-              const int64_t g = (int64_t)p * GB + 16 * warp + 8 * mi + q4;
-              if (c == 0)
-                rho_s[g] = TRI ? 2.0 * v : v;
-              else
-                drho_s[(int64_t)(c - 1) * n_pad + g] = 2.0 * v;
-            }
-            rs[c][mi] = 0.0;
-          }
+        rs[c] = 0.0;
       }
     }
   }
