@@ -110,7 +110,12 @@ kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells,
       const int n0 = jt * W, Wj = std::min(W, k8 - n0);
       for (int k0 = n0; k0 < k8; k0 += 32) {
         const int kc = std::min(32, k8 - k0);
-        frs += 2.0 * GB * kc * (double)std::min(Wj, k0 + kc - n0);
+        if (k0 < n0 + Wj) {  // diagonal chunk: rectangle before the own columns + the own block, 8-row k-step pairs m reach own groups <= m
+          const int nown = kc >> 3;
+          frs += 2.0 * GB * ((double)kc * (k0 - n0) + 32.0 * nown * (nown + 1));
+        } else {
+          frs += 2.0 * GB * kc * (double)Wj;
+        }
       }
     }
   }

@@ -72,6 +72,27 @@ __device__ __forceinline__ void rho_ksteps(double (&acc)[16][2], const double* _
   }
 }
 
+// TRI, the chunk's own (up to 4) column groups J0..: that 32x32 block of D' is itself lower triangular, so the
+// k-steps 2m, 2m+1 (chunk rows 8m..8m+7) only reach the own groups jj <= m -- 20 DMMAs instead of 32.
+template <int J0>
+__device__ __forceinline__ void rho_diag(double (&acc)[16][2], const double* __restrict__ ps,
+                                         const double* __restrict__ ds, int nown) {
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    if (m < nown) {
+#pragma unroll
+      for (int ks = 2 * m; ks < 2 * m + 2; ++ks) {
+        const double a = ps[ks * 4 * LD];
+        double b[4];
+#pragma unroll
+        for (int jj = 0; jj <= m; ++jj) b[jj] = ds[ks * 4 * (rho::NT + 4) + 8 * (J0 + jj)];
+#pragma unroll
+        for (int jj = 0; jj <= m; ++jj) dmma884(acc[J0 + jj][0], acc[J0 + jj][1], a, b[jj]);
+      }
+    }
+  }
+}
+
 // TRI epilogue of the (up to 4) column groups J0.. that became final with this chunk: the Phi columns are the
 // chunk's own first columns in the stage.  es points at column 2 r4, row 8 warp + q4 of the stage.
 template <int J0>
@@ -281,17 +302,19 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
       }
       const double* ps = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + r4 * LD + 8 * warp + q4;
       const double* ds = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + r4 * (NT + 4) + q4;
-      rho_stage(acc, ps, ds, nks, nj);
-      if (TRI) {
-        const int ecnt = h3 >> 16;
-        if (ecnt) {
-          switch ((h3 >> 10) & 3) {  // first final column group / 4
-            case 0: rho_epi_smem<0>(acc, rs[0], es, ecnt); break;
-            case 1: rho_epi_smem<4>(acc, rs[0], es, ecnt); break;
-            case 2: rho_epi_smem<8>(acc, rs[0], es, ecnt); break;
-            default: rho_epi_smem<12>(acc, rs[0], es, ecnt); break;
-          }
+      const int ecnt = TRI ? h3 >> 16 : 0;
+      if (TRI && ecnt) {
+        // diagonal chunk: rectangle of the columns before the chunk's own, then the triangular own block
+        rho_stage(acc, ps, ds, nks, (h3 >> 8) & 0xff);
+        switch ((h3 >> 10) & 3) {  // first own (= final) column group / 4
+#define KLDI_CASE(Q) \
+  case Q: rho_diag<4 * Q>(acc, ps, ds, ecnt); rho_epi_smem<4 * Q>(acc, rs[0], es, ecnt); break;
+          KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2)
+#undef KLDI_CASE
+          default: rho_diag<12>(acc, ps, ds, ecnt); rho_epi_smem<12>(acc, rs[0], es, ecnt); break;
         }
+      } else {
+        rho_stage(acc, ps, ds, nks, nj);
       }
     }
     __syncwarp();
