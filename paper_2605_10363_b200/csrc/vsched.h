@@ -28,6 +28,55 @@ struct VPass {
   int32_t max_load, units, pad0, pad1;
 };
 
+// Exact packer of one pass: the strips' column-block widths are cut into pieces of <= V_PIECE blocks and every
+// warp takes <= V_SLOTS pieces with a total load <= T.  Warps are interchangeable, so the warp being filled always
+// takes its first piece from the widest remaining strip; depth-first with a waste budget (V_WARPS*T - units) and a
+// node limit.  go() leaves the pieces per warp in out_s (strip index in `w`) / out_n (size, 0 = unused slot).
+struct VPacker {
+  int T = 0, nodes = 0;
+  std::vector<int> w;  // remaining width per strip
+  int out_s[V_WARPS][V_SLOTS], out_n[V_WARPS][V_SLOTS];
+  bool go(int warp, int remaining) {
+    static_assert(V_SLOTS == 2, "the packer fills two slots per warp");
+    if (remaining == 0) {
+      for (int v = warp; v < V_WARPS; ++v)
+        for (int k = 0; k < V_SLOTS; ++k) out_n[v][k] = 0;
+      return true;
+    }
+    if (warp == V_WARPS || ++nodes > 200000) return false;
+    const int waste = (V_WARPS - warp) * T - remaining;
+    if (waste < 0) return false;
+    int big = 0;
+    for (size_t i = 1; i < w.size(); ++i)
+      if (w[i] > w[big]) big = (int)i;
+    for (int a = std::min({V_PIECE, w[big], T}); a >= 1; --a) {
+      w[big] -= a;
+      out_s[warp][0] = big;
+      out_n[warp][0] = a;
+      for (int b = std::min(V_PIECE, T - a); b >= 0; --b) {
+        if (T - a - b > waste) break;
+        if (b == 0) {
+          out_n[warp][1] = 0;
+          if (go(warp + 1, remaining - a)) return true;
+          continue;
+        }
+        int last = -1;
+        for (size_t i = 0; i < w.size(); ++i) {
+          if (w[i] < b || w[i] == last) continue;  // strips of equal remaining width are equivalent
+          last = w[i];
+          w[i] -= b;
+          out_s[warp][1] = (int)i;
+          out_n[warp][1] = b;
+          if (go(warp + 1, remaining - a - b)) return true;
+          w[i] += b;
+        }
+      }
+      w[big] += a;
+    }
+    return false;
+  }
+};
+
 // Appends the passes of an nb-block panel to `passes` (and V_WARPS*V_SLOTS items per pass to `items`).
 inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::vector<VItem>& items) {
   const int ns = (nb + 1) / 2;
@@ -104,6 +153,41 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
           P.max_load = ml;
           P.units = units;
           std::copy(trial, trial + V_WARPS * V_SLOTS, items.begin() + item0);
+        }
+      }
+      // exact packer: smallest feasible maximum load below what longest-first found
+      {
+        std::vector<int> lo(s1 - s0), wd(s1 - s0);
+        int units = 0;
+        for (int s = s0; s < s1; ++s) {
+          lo[s - s0] = square ? j : std::max(j, 2 * s);
+          wd[s - s0] = std::max(0, j1 - lo[s - s0]);
+          units += wd[s - s0];
+        }
+        for (int T = (units + V_WARPS - 1) / V_WARPS; T < best_load; ++T) {
+          VPacker pk;
+          pk.T = T;
+          pk.w = wd;
+          if (!pk.go(0, units)) continue;
+          std::vector<int> next = lo;  // pieces of a strip are laid out left to right in warp order
+          for (int w = 0; w < V_WARPS; ++w)
+            for (int k = 0; k < V_SLOTS; ++k) {
+              VItem it{0, 0};
+              const int nj = pk.out_n[w][k];
+              if (nj) {
+                const int s = s0 + pk.out_s[w][k], j0 = next[pk.out_s[w][k]];
+                next[pk.out_s[w][k]] += nj;
+                const int a_slot = 16 * s - P.c1_lo;
+                const int b_slot = one ? 8 * j0 - P.c1_lo : P.c1_n + 8 * j0 - P.c2_lo;
+                it.a = a_slot | (b_slot << 10) | (nj << 20);
+                it.b = (16 * s) | ((8 * j0) << 16);
+              }
+              items[item0 + w * V_SLOTS + k] = it;
+            }
+          best_load = T;
+          P.max_load = T;
+          P.units = units;
+          break;
         }
       }
       passes.push_back(P);
