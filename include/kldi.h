@@ -98,7 +98,7 @@ typedef struct {
   double eps;
   double flops_rho_useful_sym; /* sum_p 128*K_p*(K_p+1): the LDA rho build, which uses D = D^T */
   double flops_rho_exec_sym;   /* FLOPs the LDA-form (triangular D) rho kernel issues */
-  double flops_v_crit;         /* V kernel: 8 warps x the busiest warp's units, summed (schedule imbalance) */
+  double flops_v_crit;         /* V kernel: 4 scheduler partitions x the busiest partition's units per pass, summed (schedule imbalance) */
   int64_t pair_stages_total;   /* KLDI_OPT_PAIR_TEST, last rho call: (K chunk, N tile) stages before the test; -1 = off */
   int64_t pair_stages_executed;/* ... and stages that contain an executable pair a_pq*b_qr >= eps (Eq. 17-19) */
 } kldi_stats;
@@ -188,7 +188,7 @@ uint64_t kldi_morton_key(const double* xyz, const double* origin);
 
 /* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
  * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32
- * {c1_lo, c1_n, c2_lo, c2_n, max_load, units, n_warps, n_slots}; items: [cap][32][2] int32 (item
+ * {c1_lo, c1_n, c2_lo, c2_n, max_load (of a warp), units, smsp_load (max over the 4 scheduler partitions w % 4), n_warps | n_slots << 8}; items: [cap][32][2] int32 (item
  * warp * n_slots + slot of the pass, the rest zero: a = a_slot | b_slot << 10 | nj << 20, b = arow | bcol << 16).  *n_passes is always set; nothing is written
  * if cap < *n_passes.  For tests of the host logic. */
 kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* items, int64_t cap, int64_t* n_passes);

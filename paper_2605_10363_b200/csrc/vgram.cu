@@ -259,7 +259,7 @@ kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const 
       vsched_build(nb, m == 1, passes, items);
       for (size_t i = ptr[nb]; i < passes.size(); ++i) {
         fexec += (double)count[nb] * passes[i].units * (2.0 * 16 * 8 * GB);
-        fcrit += (double)count[nb] * passes[i].max_load * V_WARPS * (2.0 * 16 * 8 * GB);
+        fcrit += (double)count[nb] * passes[i].smsp_load * 4 * (2.0 * 16 * 8 * GB);  // 4 scheduler partitions
       }
     }
     ptr[max_nb + 1] = (int32_t)passes.size();
@@ -468,8 +468,7 @@ kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* ite
   memset(items, 0, (size_t)*n_passes * 32 * sizeof(kldi::VItem));
   for (size_t i = 0; i < P.size(); ++i) {
     kldi::VPass q = P[i];
-    q.pad0 = kldi::V_WARPS;  // shape of the schedule, for the caller
-    q.pad1 = kldi::V_SLOTS;
+    q.pad1 = kldi::V_WARPS | (kldi::V_SLOTS << 8);  // shape of the schedule, for the caller
     memcpy(passes + 8 * i, &q, sizeof(q));
     memcpy(items + 64 * i, I.data() + i * kldi::V_ITEMS, kldi::V_ITEMS * sizeof(kldi::VItem));
   }

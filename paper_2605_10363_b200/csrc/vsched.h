@@ -25,56 +25,7 @@ struct VItem {      // one slot of one consumer warp in one pass
 };
 struct VPass {
   int32_t c1_lo, c1_n, c2_lo, c2_n;  // packed column intervals streamed into the stage (interval 2 may be empty)
-  int32_t max_load, units, pad0, pad1;
-};
-
-// Exact packer of one pass: the strips' column-block widths are cut into pieces of <= V_PIECE blocks and every
-// warp takes <= V_SLOTS pieces with a total load <= T.  Warps are interchangeable, so the warp being filled always
-// takes its first piece from the widest remaining strip; depth-first with a waste budget (V_WARPS*T - units) and a
-// node limit.  go() leaves the pieces per warp in out_s (strip index in `w`) / out_n (size, 0 = unused slot).
-struct VPacker {
-  int T = 0, nodes = 0;
-  std::vector<int> w;  // remaining width per strip
-  int out_s[V_WARPS][V_SLOTS], out_n[V_WARPS][V_SLOTS];
-  bool go(int warp, int remaining) {
-    static_assert(V_SLOTS == 2, "the packer fills two slots per warp");
-    if (remaining == 0) {
-      for (int v = warp; v < V_WARPS; ++v)
-        for (int k = 0; k < V_SLOTS; ++k) out_n[v][k] = 0;
-      return true;
-    }
-    if (warp == V_WARPS || ++nodes > 200000) return false;
-    const int waste = (V_WARPS - warp) * T - remaining;
-    if (waste < 0) return false;
-    int big = 0;
-    for (size_t i = 1; i < w.size(); ++i)
-      if (w[i] > w[big]) big = (int)i;
-    for (int a = std::min({V_PIECE, w[big], T}); a >= 1; --a) {
-      w[big] -= a;
-      out_s[warp][0] = big;
-      out_n[warp][0] = a;
-      for (int b = std::min(V_PIECE, T - a); b >= 0; --b) {
-        if (T - a - b > waste) break;
-        if (b == 0) {
-          out_n[warp][1] = 0;
-          if (go(warp + 1, remaining - a)) return true;
-          continue;
-        }
-        int last = -1;
-        for (size_t i = 0; i < w.size(); ++i) {
-          if (w[i] < b || w[i] == last) continue;  // strips of equal remaining width are equivalent
-          last = w[i];
-          w[i] -= b;
-          out_s[warp][1] = (int)i;
-          out_n[warp][1] = b;
-          if (go(warp + 1, remaining - a - b)) return true;
-          w[i] += b;
-        }
-      }
-      w[big] += a;
-    }
-    return false;
-  }
+  int32_t max_load, units, smsp_load, pad1;  // max load of a warp / of a scheduler partition (warps w % 4), in units
 };
 
 // Appends the passes of an nb-block panel to `passes` (and V_WARPS*V_SLOTS items per pass to `items`).
@@ -118,11 +69,17 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
         P.c2_lo = 8 * j;
         P.c2_n = 8 * (j1 - j);
       }
-      // pieces: try piece widths 4..1 and keep the assignment with the smallest maximum warp load
+      // Pieces -> warps.  The FP64 tensor pipe belongs to a scheduler partition (SMSP = warp % 4), and 15 consumer
+      // warps leave partition 3 with three of them (the producer is the fourth), so the quantity to balance is the
+      // load per partition, not per warp: pieces are spread longest-first over the four partitions (slot limits
+      // 2 x warps of the partition), then pieces of the fullest partition are moved or split towards the emptiest
+      // while that lowers the maximum, and each partition deals its pieces to its own warps.
       struct Piece { int s, j0, nj; };
       const size_t item0 = items.size();
       items.resize(item0 + V_ITEMS, VItem{0, 0});
-      int best_load = 1 << 30;
+      int nwq[4] = {0, 0, 0, 0};
+      for (int w = 0; w < V_WARPS; ++w) nwq[w & 3]++;
+      int best_q = 1 << 30, best_w = 1 << 30;
       for (int pw = V_PIECE; pw >= 1; --pw) {
         std::vector<Piece> pc;
         for (int s = s0; s < s1; ++s) {
@@ -131,63 +88,77 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
         }
         if ((int)pc.size() > V_WARPS * V_SLOTS) break;
         std::stable_sort(pc.begin(), pc.end(), [](const Piece& x, const Piece& y) { return x.nj > y.nj; });
-        int load[V_WARPS] = {0}, used[V_WARPS] = {0};
-        VItem trial[V_WARPS * V_SLOTS] = {};
-        int units = 0;
+        std::vector<Piece> bin[4];
+        int load[4] = {0, 0, 0, 0};
+        bool ok = true;
         for (const Piece& q : pc) {
           int best = -1;
-          for (int w = 0; w < V_WARPS; ++w)
-            if (used[w] < V_SLOTS && (best < 0 || load[w] < load[best])) best = w;
-          const int a_slot = 16 * q.s - P.c1_lo;
-          const int b_slot = one ? 8 * q.j0 - P.c1_lo : P.c1_n + 8 * q.j0 - P.c2_lo;
-          VItem& it = trial[best * V_SLOTS + used[best]];
-          it.a = a_slot | (b_slot << 10) | (q.nj << 20);
-          it.b = (16 * q.s) | ((8 * q.j0) << 16);
+          for (int b = 0; b < 4; ++b)
+            if ((int)bin[b].size() < V_SLOTS * nwq[b] && (best < 0 || load[b] < load[best])) best = b;
+          if (best < 0) { ok = false; break; }
+          bin[best].push_back(q);
           load[best] += q.nj;
-          used[best]++;
-          units += q.nj;
         }
-        const int ml = *std::max_element(load, load + V_WARPS);
-        if (ml < best_load) {
-          best_load = ml;
-          P.max_load = ml;
+        if (!ok) continue;
+        for (int iter = 0; iter < 64; ++iter) {  // move / split from the fullest to the emptiest partition
+          int hi = 0, lo = 0;
+          for (int b = 1; b < 4; ++b) {
+            if (load[b] > load[hi]) hi = b;
+            if (load[b] < load[lo]) lo = b;
+          }
+          const int gap = load[hi] - load[lo];
+          if (gap < 2 || (int)bin[lo].size() >= V_SLOTS * nwq[lo]) break;
+          const int want = gap / 2;
+          int pick = -1;  // largest piece not larger than want, else any piece to split
+          for (size_t i = 0; i < bin[hi].size(); ++i)
+            if (bin[hi][i].nj <= want && (pick < 0 || bin[hi][i].nj > bin[hi][pick].nj)) pick = (int)i;
+          if (pick >= 0) {
+            bin[lo].push_back(bin[hi][pick]);
+            load[lo] += bin[hi][pick].nj;
+            load[hi] -= bin[hi][pick].nj;
+            bin[hi].erase(bin[hi].begin() + pick);
+            continue;
+          }
+          for (size_t i = 0; i < bin[hi].size(); ++i)
+            if (bin[hi][i].nj > want) { pick = (int)i; break; }
+          if (pick < 0) break;
+          Piece& src = bin[hi][pick];
+          src.nj -= want;
+          bin[lo].push_back({src.s, src.j0 + src.nj, want});
+          load[hi] -= want;
+          load[lo] += want;
+        }
+        const int mq = *std::max_element(load, load + 4);
+        // deal the pieces of a partition to its warps: largest first, then back in reverse order
+        VItem trial[V_WARPS * V_SLOTS] = {};
+        int wload[V_WARPS] = {0};
+        int units = 0;
+        for (int b = 0; b < 4; ++b) {
+          std::stable_sort(bin[b].begin(), bin[b].end(), [](const Piece& x, const Piece& y) { return x.nj > y.nj; });
+          int used[(V_WARPS + 3) / 4] = {0};
+          for (const Piece& q : bin[b]) {
+            int bw = -1;
+            for (int i = 0; i < nwq[b]; ++i)
+              if (used[i] < V_SLOTS && (bw < 0 || wload[b + 4 * i] < wload[b + 4 * bw])) bw = i;
+            const int w = b + 4 * bw;
+            const int a_slot = 16 * q.s - P.c1_lo;
+            const int b_slot = one ? 8 * q.j0 - P.c1_lo : P.c1_n + 8 * q.j0 - P.c2_lo;
+            VItem& it = trial[w * V_SLOTS + used[bw]];
+            it.a = a_slot | (b_slot << 10) | (q.nj << 20);
+            it.b = (16 * q.s) | ((8 * q.j0) << 16);
+            wload[w] += q.nj;
+            used[bw]++;
+            units += q.nj;
+          }
+        }
+        const int mw = *std::max_element(wload, wload + V_WARPS);
+        if (mq < best_q || (mq == best_q && mw < best_w)) {
+          best_q = mq;
+          best_w = mw;
+          P.max_load = mw;
+          P.smsp_load = mq;
           P.units = units;
           std::copy(trial, trial + V_WARPS * V_SLOTS, items.begin() + item0);
-        }
-      }
-      // exact packer: smallest feasible maximum load below what longest-first found
-      {
-        std::vector<int> lo(s1 - s0), wd(s1 - s0);
-        int units = 0;
-        for (int s = s0; s < s1; ++s) {
-          lo[s - s0] = square ? j : std::max(j, 2 * s);
-          wd[s - s0] = std::max(0, j1 - lo[s - s0]);
-          units += wd[s - s0];
-        }
-        for (int T = (units + V_WARPS - 1) / V_WARPS; T < best_load; ++T) {
-          VPacker pk;
-          pk.T = T;
-          pk.w = wd;
-          if (!pk.go(0, units)) continue;
-          std::vector<int> next = lo;  // pieces of a strip are laid out left to right in warp order
-          for (int w = 0; w < V_WARPS; ++w)
-            for (int k = 0; k < V_SLOTS; ++k) {
-              VItem it{0, 0};
-              const int nj = pk.out_n[w][k];
-              if (nj) {
-                const int s = s0 + pk.out_s[w][k], j0 = next[pk.out_s[w][k]];
-                next[pk.out_s[w][k]] += nj;
-                const int a_slot = 16 * s - P.c1_lo;
-                const int b_slot = one ? 8 * j0 - P.c1_lo : P.c1_n + 8 * j0 - P.c2_lo;
-                it.a = a_slot | (b_slot << 10) | (nj << 20);
-                it.b = (16 * s) | ((8 * j0) << 16);
-              }
-              items[item0 + w * V_SLOTS + k] = it;
-            }
-          best_load = T;
-          P.max_load = T;
-          P.units = units;
-          break;
         }
       }
       passes.push_back(P);

@@ -120,7 +120,8 @@ def test_v_schedule_covers_every_unit_once(square):
         ns = (nb + 1) // 2
         seen = np.zeros((ns, nb), dtype=np.int32)
         for P, I in zip(passes, items):
-            c1_lo, c1_n, c2_lo, c2_n, max_load, units, n_warps, n_slots = (int(v) for v in P[:8])
+            c1_lo, c1_n, c2_lo, c2_n, max_load, units, smsp_load, shape = (int(v) for v in P[:8])
+            n_warps, n_slots = shape & 0xFF, shape >> 8
             assert n_warps * n_slots <= 32
             assert c1_n + c2_n <= 256 and c1_lo % 8 == 0 and c2_lo % 8 == 0 and c1_n % 8 == 0 and c2_n % 8 == 0
             loads, tot = [], 0
@@ -147,6 +148,9 @@ def test_v_schedule_covers_every_unit_once(square):
                 loads.append(load)
                 tot += load
             assert max(loads) == max_load <= 4 * n_slots and tot == units
+            # the balanced quantity: load per scheduler partition (warp % 4 shares one FP64 tensor pipe)
+            assert max(sum(loads[q::4]) for q in range(4)) == smsp_load
+            assert 4 * smsp_load <= units + 4 * 4 + 3 or n_warps * n_slots < 16
         want = np.ones((ns, nb), dtype=np.int32)
         if not square:
             for s in range(ns):
