@@ -178,7 +178,8 @@ typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2 } kldi_optio
 kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
 
 /* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`
- * iterations; returns achieved TFLOP/s (device-timed) in *tflops.  kind 0 = DMMA, 1 = DFMA. */
+ * iterations; returns achieved TFLOP/s (device-timed) in *tflops.  kind 0 = DMMA, 1 = DFMA,
+ * 2 = 16 DMMA + 64 DFMA per iteration (do the tensor and the vector FP64 instructions share a pipe?). */
 kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);
 
 /* Eq. 20 as the plan applies it, on the host, no GPU needed: the 60-bit key
@@ -189,7 +190,7 @@ uint64_t kldi_morton_key(const double* xyz, const double* origin);
 /* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
  * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32
  * {c1_lo, c1_n, c2_lo, c2_n, max_load (of a warp), units, smsp_load (max over the 4 scheduler partitions w % 4), n_warps | n_slots << 8}; items: [cap][32][2] int32 (item
- * warp * n_slots + slot of the pass, the rest zero: a = a_slot | b_slot << 10 | nj << 20, b = arow | bcol << 16).  *n_passes is always set; nothing is written
+ * warp * n_slots + slot of the pass, the rest zero: a = a_slot | b_slot << 10 | nj << 20 | diag << 24, b = arow | bcol << 16; loads and units count 8x8 blocks).  *n_passes is always set; nothing is written
  * if cap < *n_passes.  For tests of the host logic. */
 kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* items, int64_t cap, int64_t* n_passes);
 

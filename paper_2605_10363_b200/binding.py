@@ -276,5 +276,5 @@ def vlayout_offset(panel_off: int, K8: int, col: int, row: int) -> int:
 
 def fp64_peak(kind: str = "dmma", iters: int = 20000) -> float:
     t = C.c_double(0.0)
-    _check(lib().kldi_fp64_peak(0 if kind == "dmma" else 1, int(iters), C.byref(t)), "kldi_fp64_peak")
+    _check(lib().kldi_fp64_peak({"dmma": 0, "dfma": 1, "mix": 2}[kind], int(iters), C.byref(t)), "kldi_fp64_peak")
     return t.value

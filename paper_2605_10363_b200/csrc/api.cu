@@ -46,6 +46,25 @@ __global__ void __launch_bounds__(256) k_peak_dfma(int iters, double* sink) {
   for (int i = 0; i < 16; ++i) s += c[i];
   if (s == 123.456) sink[0] = s;
 }
+// 16 DMMA + 64 DFMA per iteration: tells whether the tensor and the vector FP64 instructions share one pipe
+__global__ void __launch_bounds__(256) k_peak_mix(int iters, double* sink) {
+  double c[16][2], f[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) { c[i][0] = c[i][1] = 0.0; f[i] = i; }
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      dmma884(c[i][0], c[i][1], a, b);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) f[(4 * i + r) & 15] = fma(f[(4 * i + r) & 15], a, b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1] + f[i];
+  if (s == 123.456) sink[0] = s;
+}
 }  // namespace kldi
 
 using namespace kldi;
@@ -384,14 +403,18 @@ kldi_status kldi_fp64_peak(int kind, int iters, double* tflops) {
     KLDI_CUDA(cudaEventRecord(e0));
     if (kind == 0)
       k_peak_dmma<<<grid, 256>>>(iters, sink);
-    else
+    else if (kind == 1)
       k_peak_dfma<<<grid, 256>>>(iters, sink);
+    else
+      k_peak_mix<<<grid, 256>>>(iters, sink);
     KLDI_CUDA(cudaEventRecord(e1));
     KLDI_CUDA(cudaEventSynchronize(e1));
   }
   float ms = 0.f;
   KLDI_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-  const double per_thread_block = (kind == 0) ? 8.0 * 16 * 2 * 8 * 8 * 4 : 256.0 * 16 * 2;  // flops per CTA per iter
+  const double per_thread_block = (kind == 0)   ? 8.0 * 16 * 2 * 8 * 8 * 4
+                                  : (kind == 1) ? 256.0 * 16 * 2
+                                                : 8.0 * 16 * 2 * 8 * 8 * 4 + 256.0 * 64 * 2;  // flops per CTA per iter
   *tflops = per_thread_block * iters * grid / (ms * 1e-3) / 1e12;
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);

@@ -29,7 +29,9 @@ enum { F_FIRST = 1, F_LAST = 2, F_DONE = 4 };
 
 // One slab (32 grid rows = 8 k-steps) of one item.  A, B point at the item's first column (+ q4 columns);
 // o0/o1 are the lane's swizzled offsets of chunks 2 r4 and 2 r4 + 1; a 16-byte load feeds two k-steps.
-template <int NJ, bool GGA>
+// DIAG: the item's first block sits on the diagonal of an LDA strip; its rows 8..15 lie strictly below it and are
+// skipped (acc[1][0] stays zero and is never written back).
+template <int NJ, bool GGA, bool DIAG>
 __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __restrict__ A,
                                        const double* __restrict__ B, const double* __restrict__ w, int o0, int o1) {
   using namespace vg;
@@ -51,12 +53,12 @@ __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __r
 #pragma unroll
       for (int n = 0; n < NJ; ++n) {
         dmma884(acc[0][n][0], acc[0][n][1], a0.x, b[n].x);
-        dmma884(acc[1][n][0], acc[1][n][1], a1.x, b[n].x);
+        if (!(DIAG && n == 0)) dmma884(acc[1][n][0], acc[1][n][1], a1.x, b[n].x);
       }
 #pragma unroll
       for (int n = 0; n < NJ; ++n) {
         dmma884(acc[0][n][0], acc[0][n][1], a0.y, b[n].y);
-        dmma884(acc[1][n][0], acc[1][n][1], a1.y, b[n].y);
+        if (!(DIAG && n == 0)) dmma884(acc[1][n][0], acc[1][n][1], a1.y, b[n].y);
       }
     }
   }
@@ -167,14 +169,17 @@ __global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
     const double* wb = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + COLS_BYTES) + 4 * r4;
 #pragma unroll
     for (int k = 0; k < V_SLOTS; ++k) {
-      const int nj = ia[k] >> 20;
       const double* A = st + (ia[k] & 1023) * STR;
       const double* B = st + ((ia[k] >> 10) & 1023) * STR;
-      switch (nj) {
-        case 1: vg_run<1, GGA>(acc[k], A, B, wb, o0, o1); break;
-        case 2: vg_run<2, GGA>(acc[k], A, B, wb, o0, o1); break;
-        case 3: vg_run<3, GGA>(acc[k], A, B, wb, o0, o1); break;
-        case 4: vg_run<4, GGA>(acc[k], A, B, wb, o0, o1); break;
+      switch (ia[k] >> 20) {  // nj | diag << 4
+        case 1: vg_run<1, GGA, false>(acc[k], A, B, wb, o0, o1); break;
+        case 2: vg_run<2, GGA, false>(acc[k], A, B, wb, o0, o1); break;
+        case 3: vg_run<3, GGA, false>(acc[k], A, B, wb, o0, o1); break;
+        case 4: vg_run<4, GGA, false>(acc[k], A, B, wb, o0, o1); break;
+        case 17: if (!GGA) vg_run<1, GGA, true>(acc[k], A, B, wb, o0, o1); break;
+        case 18: if (!GGA) vg_run<2, GGA, true>(acc[k], A, B, wb, o0, o1); break;
+        case 19: if (!GGA) vg_run<3, GGA, true>(acc[k], A, B, wb, o0, o1); break;
+        case 20: if (!GGA) vg_run<4, GGA, true>(acc[k], A, B, wb, o0, o1); break;
         default: break;
       }
     }
@@ -189,7 +194,7 @@ __global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
     if (fl & F_LAST) {
 #pragma unroll
       for (int k = 0; k < V_SLOTS; ++k) {
-        const int nj = ia[k] >> 20;
+        const int nj = (ia[k] >> 20) & 7;
         if (nj == 0) continue;
         const int arow = ib[k] & 0xffff, bcol = ib[k] >> 16;
 #pragma unroll
@@ -258,8 +263,8 @@ kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const 
       if (nb == 0 || count[nb] == 0) continue;
       vsched_build(nb, m == 1, passes, items);
       for (size_t i = ptr[nb]; i < passes.size(); ++i) {
-        fexec += (double)count[nb] * passes[i].units * (2.0 * 16 * 8 * GB);
-        fcrit += (double)count[nb] * passes[i].smsp_load * 4 * (2.0 * 16 * 8 * GB);  // 4 scheduler partitions
+        fexec += (double)count[nb] * passes[i].units * (2.0 * 8 * 8 * GB);  // units: 8x8 blocks
+        fcrit += (double)count[nb] * passes[i].smsp_load * 4 * (2.0 * 8 * 8 * GB);  // 4 scheduler partitions
       }
     }
     ptr[max_nb + 1] = (int32_t)passes.size();

@@ -20,12 +20,14 @@ constexpr int V_WARPS = 15, V_SLOTS = 2, V_PIECE = 4, V_BAND = 8, V_MAXCOLS = 25
 constexpr int V_ITEMS = (V_WARPS * V_SLOTS + 1) & ~1;  // VItems stored per pass (even: 16-byte bulk copies)
 
 struct VItem {      // one slot of one consumer warp in one pass
-  int32_t a;        // a_slot | b_slot << 10 | nj << 20   (stage-buffer column slots, nj = column blocks)
+  int32_t a;        // a_slot | b_slot << 10 | nj << 20 | diag << 24  (stage-buffer column slots, nj = column blocks,
+                    // diag: the item starts on the diagonal, rows 8..15 of its first block are not computed)
   int32_t b;        // arow | bcol << 16                  (packed row / column of the item's first element)
 };
 struct VPass {
   int32_t c1_lo, c1_n, c2_lo, c2_n;  // packed column intervals streamed into the stage (interval 2 may be empty)
-  int32_t max_load, units, smsp_load, pad1;  // max load of a warp / of a scheduler partition (warps w % 4), in units
+  int32_t max_load, units, smsp_load, pad1;  // max load of a warp / of a scheduler partition (warps w % 4) and the
+                                             // pass total, in 8x8 blocks (one DMMA per k-step each)
 };
 
 // Appends the passes of an nb-block panel to `passes` (and V_WARPS*V_SLOTS items per pass to `items`).
@@ -74,7 +76,12 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
       // load per partition, not per warp: pieces are spread longest-first over the four partitions (slot limits
       // 2 x warps of the partition), then pieces of the fullest partition are moved or split towards the emptiest
       // while that lowers the maximum, and each partition deals its pieces to its own warps.
-      struct Piece { int s, j0, nj; };
+      // cost of a piece in 8x8 blocks (= DMMAs per k-step): 2 per column block, minus the lower 8 rows of the strip's
+      // first block on the diagonal, which lie strictly below it and are not computed (VItem diag flag)
+      struct Piece {
+        int s, j0, nj, diag;
+        int cost() const { return 2 * nj - diag; }
+      };
       const size_t item0 = items.size();
       items.resize(item0 + V_ITEMS, VItem{0, 0});
       int nwq[4] = {0, 0, 0, 0};
@@ -84,10 +91,10 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
         std::vector<Piece> pc;
         for (int s = s0; s < s1; ++s) {
           const int lo = square ? j : std::max(j, 2 * s);
-          for (int c = lo; c < j1; c += pw) pc.push_back({s, c, std::min(pw, j1 - c)});
+          for (int c = lo; c < j1; c += pw) pc.push_back({s, c, std::min(pw, j1 - c), (!square && c == 2 * s) ? 1 : 0});
         }
         if ((int)pc.size() > V_WARPS * V_SLOTS) break;
-        std::stable_sort(pc.begin(), pc.end(), [](const Piece& x, const Piece& y) { return x.nj > y.nj; });
+        std::stable_sort(pc.begin(), pc.end(), [](const Piece& x, const Piece& y) { return x.cost() > y.cost(); });
         std::vector<Piece> bin[4];
         int load[4] = {0, 0, 0, 0};
         bool ok = true;
@@ -97,7 +104,7 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
             if ((int)bin[b].size() < V_SLOTS * nwq[b] && (best < 0 || load[b] < load[best])) best = b;
           if (best < 0) { ok = false; break; }
           bin[best].push_back(q);
-          load[best] += q.nj;
+          load[best] += q.cost();
         }
         if (!ok) continue;
         for (int iter = 0; iter < 64; ++iter) {  // move / split from the fullest to the emptiest partition
@@ -108,25 +115,27 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
           }
           const int gap = load[hi] - load[lo];
           if (gap < 2 || (int)bin[lo].size() >= V_SLOTS * nwq[lo]) break;
-          const int want = gap / 2;
+          const int want = gap / 2;  // in 8x8 blocks
           int pick = -1;  // largest piece not larger than want, else any piece to split
           for (size_t i = 0; i < bin[hi].size(); ++i)
-            if (bin[hi][i].nj <= want && (pick < 0 || bin[hi][i].nj > bin[hi][pick].nj)) pick = (int)i;
+            if (bin[hi][i].cost() <= want && (pick < 0 || bin[hi][i].cost() > bin[hi][pick].cost())) pick = (int)i;
           if (pick >= 0) {
             bin[lo].push_back(bin[hi][pick]);
-            load[lo] += bin[hi][pick].nj;
-            load[hi] -= bin[hi][pick].nj;
+            load[lo] += bin[hi][pick].cost();
+            load[hi] -= bin[hi][pick].cost();
             bin[hi].erase(bin[hi].begin() + pick);
             continue;
           }
+          const int cut = want / 2;  // whole column blocks split off the tail of a piece (the diag flag stays in front)
+          if (cut < 1) break;
           for (size_t i = 0; i < bin[hi].size(); ++i)
-            if (bin[hi][i].nj > want) { pick = (int)i; break; }
+            if (bin[hi][i].nj > cut) { pick = (int)i; break; }
           if (pick < 0) break;
           Piece& src = bin[hi][pick];
-          src.nj -= want;
-          bin[lo].push_back({src.s, src.j0 + src.nj, want});
-          load[hi] -= want;
-          load[lo] += want;
+          src.nj -= cut;
+          bin[lo].push_back({src.s, src.j0 + src.nj, cut, 0});
+          load[hi] -= 2 * cut;
+          load[lo] += 2 * cut;
         }
         const int mq = *std::max_element(load, load + 4);
         // deal the pieces of a partition to its warps: largest first, then back in reverse order
@@ -134,7 +143,7 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
         int wload[V_WARPS] = {0};
         int units = 0;
         for (int b = 0; b < 4; ++b) {
-          std::stable_sort(bin[b].begin(), bin[b].end(), [](const Piece& x, const Piece& y) { return x.nj > y.nj; });
+          std::stable_sort(bin[b].begin(), bin[b].end(), [](const Piece& x, const Piece& y) { return x.cost() > y.cost(); });
           int used[(V_WARPS + 3) / 4] = {0};
           for (const Piece& q : bin[b]) {
             int bw = -1;
@@ -144,11 +153,11 @@ inline void vsched_build(int nb, bool square, std::vector<VPass>& passes, std::v
             const int a_slot = 16 * q.s - P.c1_lo;
             const int b_slot = one ? 8 * q.j0 - P.c1_lo : P.c1_n + 8 * q.j0 - P.c2_lo;
             VItem& it = trial[w * V_SLOTS + used[bw]];
-            it.a = a_slot | (b_slot << 10) | (q.nj << 20);
+            it.a = a_slot | (b_slot << 10) | (q.nj << 20) | (q.diag << 24);
             it.b = (16 * q.s) | ((8 * q.j0) << 16);
-            wload[w] += q.nj;
+            wload[w] += q.cost();
             used[bw]++;
-            units += q.nj;
+            units += q.cost();
           }
         }
         const int mw = *std::max_element(wload, wload + V_WARPS);

@@ -129,7 +129,7 @@ def test_v_schedule_covers_every_unit_once(square):
                 load = 0
                 for k in range(n_slots):
                     a, b = int(I[w * n_slots + k, 0]), int(I[w * n_slots + k, 1])
-                    nj, a_slot, b_slot = a >> 20, a & 1023, (a >> 10) & 1023
+                    nj, diag, a_slot, b_slot = (a >> 20) & 7, (a >> 24) & 1, a & 1023, (a >> 10) & 1023
                     if nj == 0:
                         continue
                     assert 1 <= nj <= 4
@@ -144,13 +144,15 @@ def test_v_schedule_covers_every_unit_once(square):
                     s = arow // 16
                     for j in range(bcol // 8, bcol // 8 + nj):
                         seen[s, j] += 1
-                    load += nj
+                    # diag: the lower 8 rows of a strip's first block on the diagonal are not computed (LDA only)
+                    assert diag == (0 if square else int(bcol == arow))
+                    load += 2 * nj - diag
                 loads.append(load)
                 tot += load
-            assert max(loads) == max_load <= 4 * n_slots and tot == units
+            assert max(loads) == max_load <= 2 * 4 * n_slots and tot == units    # in 8x8 blocks
             # the balanced quantity: load per scheduler partition (warp % 4 shares one FP64 tensor pipe)
             assert max(sum(loads[q::4]) for q in range(4)) == smsp_load
-            assert 4 * smsp_load <= units + 4 * 4 + 3 or n_warps * n_slots < 16
+            assert 4 * smsp_load <= units + 4 * 8 + 3
         want = np.ones((ns, nb), dtype=np.int32)
         if not square:
             for s in range(ns):
