@@ -21,7 +21,8 @@ dense-product step; `brute_force_lda` below is the same thing as explicit Python
 
 Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): analytic Gaussian overlap => diag(S)=1 and
 int rho = Tr(D S); closed-form Slater energy of one s-Gaussian; V symmetric; central finite
-differences dE/dD = V (LDA and PBE-x); brute-force loops on single water; PBE-x limits.
+differences dE/dD = V (LDA and PBE-x); brute-force loops on single water; PBE-x limits; central finite
+differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda.
 Absolute PBE-x energies have no printed reference value: beyond the limits and the FD
 identity they are "parity unpinned".
 """
@@ -222,6 +223,35 @@ def exc_energy_from_rho(w, rho, drho=None, functional: str = "lda") -> float:
     else:
         e, _ = slater(rho)
     return math.fsum((np.asarray(w) * e).tolist())
+
+
+# ----------------------------------------------------------------------------- nuclear gradient
+def exc_nuclear_gradient_lda(basis, pts, w, D, chunk: int = 8192):
+    """EXC nuclear-gradient contraction, LDA, at fixed density matrix and FIXED quadrature (points and weights do not
+    move with the atoms: no grid response) — the paper's second workload, for which it prints no
+    formula; this is the chain rule on E_xc = sum_g w_g e(rho_g) written out (G1):
+
+        chi_mu depends on the nucleus A it sits on through r - A  =>  d chi_mu(r_g) / d A_c = - d_c chi_mu(r_g),
+        d rho_g / d A_c = -2 sum_{mu on A} d_c chi_mu(r_g) X_{g,mu},   X = Phi D  (D symmetric, Eq. 4),
+        dE_xc / d A_c   = sum_g w_g v_rho(rho_g) d rho_g / d A_c
+                        = -2 sum_g w_g v_g sum_{mu on A} d_c Phi_{g,mu} X_{g,mu}.
+
+    Returns grad [n_atoms][3].  Pinned by central finite differences of the oracle's own energy in the atom
+    coordinates with the same points and weights (tests/test_oracle_pins.py)."""
+    atom_xyz, shell_atom, shell_l = basis[0], basis[1], basis[2]
+    ao_atom = np.concatenate([[int(shell_atom[s])] * ((int(l) + 1) * (int(l) + 2) // 2) for s, l in enumerate(shell_l)])
+    n_atoms = len(atom_xyz)
+    grad = np.zeros((n_atoms, 3))
+    for c0 in range(0, len(pts), chunk):
+        phi, dphi = ao_values(*basis, pts[c0:c0 + chunk], deriv=True)
+        rho = density(phi, D)
+        _, v = slater(rho)
+        wv = w[c0:c0 + chunk] * v
+        X = phi @ D
+        for c in range(3):
+            per_ao = -2.0 * np.einsum("g,gm,gm->m", wv, dphi[c], X)
+            np.add.at(grad[:, c], ao_atom, per_ao)
+    return grad
 
 
 # ----------------------------------------------------------------------------- sampled entries

@@ -131,6 +131,30 @@ def test_ao_gradient_matches_finite_difference(water):
         assert np.max(np.abs(fd - drho[c])) < 1e-7
 
 
+def test_nuclear_gradient_lda_matches_finite_difference_of_energy(water):
+    """the paper prints no gradient formula, so the oracle's EXC nuclear-gradient contraction is
+    pinned by central differences of the (closed-form-pinned) energy in the atom coordinates, grid held fixed, and
+    by the translation identity sum_A dE/dA_c = -sum_g w_g v_g d_c rho_g (moving every atom = moving the grid back)."""
+    basis = basis_of(water)
+    g = O.exc_nuclear_gradient_lda(basis, water.grid_xyz, water.grid_w, water.D)
+    assert g.shape == (3, 3) and np.max(np.abs(g)) > 1e-3
+    h = 1e-4
+    for (a, c) in [(0, 0), (0, 2), (1, 1), (2, 0), (2, 2)]:
+        e = []
+        for sgn in (+1, -1):
+            xyz = np.array(basis[0], dtype=np.float64, copy=True)
+            xyz[a, c] += sgn * h
+            e.append(O.exc((xyz,) + tuple(basis[1:]), water.grid_xyz, water.grid_w, water.D, "lda", want_v=False)["E"])
+        fd = (e[0] - e[1]) / (2 * h)
+        assert abs(fd - g[a, c]) < 1e-6 * np.max(np.abs(g)), (a, c, fd, g[a, c])
+    phi, dphi = O.ao_values(*basis, water.grid_xyz, deriv=True)
+    rho = O.density(phi, water.D)
+    drho = O.density_gradient(phi, dphi, water.D)
+    wv = water.grid_w * O.slater(rho)[1]
+    for c in range(3):
+        assert abs(g[:, c].sum() + np.dot(wv, drho[c])) < 1e-10 * np.max(np.abs(g))
+
+
 def test_pbe_enhancement_limits():
     rho = np.geomspace(1e-12, 50.0, 200)
     e_s, v_s = O.slater(rho)
