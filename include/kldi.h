@@ -165,6 +165,17 @@ kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_
 kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, double* out,
                                   int64_t cap_bytes, int32_t* width);
 
+/* EXC nuclear-gradient contraction (the paper's second workload; it prints no formula, so this is
+ * the chain rule on E_xc = sum_g w_g e(rho_g), DESIGN.md §3 reading G1): at fixed D and FIXED quadrature (points and
+ * weights do not follow the atoms, no grid response),
+ *     grad[A][c] = dE_xc/dA_c = -2 sum_g w_g v_rho(rho_g) sum_{mu on A} d_c Phi_{g,mu} X_{g,mu},   X = Phi D,
+ * over the retained (grid-block, AO-shell) pairs.  LDA only (f = KLDI_LDA_SLATER; anything else -> KLDI_EINVAL); the
+ * plan must hold the gradient stores (want_gradients = 1, else KLDI_ESTATE).  D: DEVICE [n_ao][n_ao] row-major,
+ * symmetric.  grad: DEVICE [n_atoms][3], caller atom order, overwritten.  Exc: HOST, may be NULL.  The first call
+ * allocates an X store of the size of one Phi store, owned by the plan.  Synchronises before it returns.
+ * kldi_last_timings: rho = the X / rho build, vxc = the gradient contraction. */
+kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, double* Exc, double* grad);
+
 /* Options of a plan (kldi_plan_set_option returns KLDI_EINVAL for an unknown option).
  * KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram tile into V with
  * red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a workspace (allocated on

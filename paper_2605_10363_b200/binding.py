@@ -20,7 +20,7 @@ KLDI_GGA_PBEX = 1
 
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
-    "kldi_exc_host", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
+    "kldi_exc_host", "kldi_exc_grad", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
     "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
     "kldi_vlayout_offset",
 ]
@@ -81,6 +81,7 @@ def lib():
         L.kldi_build_vxc.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.kldi_exc.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_exc_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        L.kldi_exc_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_last_timings.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.kldi_plan_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_plan_export_tile.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_int64,
@@ -209,6 +210,16 @@ class Plan:
         _check(lib().kldi_exc(self._h, self._dev64(D, (self.n_ao, self.n_ao), "D"), int(functional), C.byref(e),
                               self._dev64(V, (self.n_ao, self.n_ao), "V") if want_v else None), "kldi_exc")
         return e.value, V
+
+    def exc_grad(self, D, functional: int = KLDI_LDA_SLATER):
+        """kldi_exc_grad: (E_xc, grad [n_atoms][3] device tensor, caller atom order)."""
+        import torch
+
+        g = torch.empty((int(self.stats.n_atoms), 3), dtype=torch.float64, device=self.device)
+        e = C.c_double(0.0)
+        _check(lib().kldi_exc_grad(self._h, self._dev64(D, (self.n_ao, self.n_ao), "D"), int(functional), C.byref(e),
+                                   C.c_void_p(g.data_ptr())), "kldi_exc_grad")
+        return e.value, g
 
     def exc_host(self, D_host, functional: int = KLDI_LDA_SLATER, V_host=None):
         """End-to-end form: D_host / V_host are host float64 arrays (numpy or pinned torch CPU tensors)."""

@@ -277,6 +277,40 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
   return KLDI_OK;
 }
 
+kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, double* Exc, double* grad) {
+  if (!P || !D || !grad) {
+    set_error("kldi_exc_grad: null argument");
+    return KLDI_EINVAL;
+  }
+  if (f != KLDI_LDA_SLATER) {
+    set_error("kldi_exc_grad: only KLDI_LDA_SLATER is built (a GGA gradient needs the AO second derivatives)");
+    return KLDI_EINVAL;
+  }
+  if (!P->want_grad) {
+    set_error("kldi_exc_grad: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
+    return KLDI_ESTATE;
+  }
+  if (!P->d_x) KLDI_CUDA(cudaMalloc(&P->d_x, sizeof(double) * GB * (size_t)(P->total_cols + 64)));
+  kldi_status rc;
+  P->have_timings = false;
+  EV(0);
+  if ((rc = launch_permute_D(P, D, true)) != KLDI_OK) return rc;  // full D: the gradient needs X = Phi D itself
+  EV(1);
+  if ((rc = launch_rho(P, true, P->d_x)) != KLDI_OK) return rc;
+  EV(2);
+  if ((rc = launch_xc(P, f)) != KLDI_OK) return rc;
+  EV(3);
+  EV(4);
+  if ((rc = launch_grad_cols(P, grad)) != KLDI_OK) return rc;
+  EV(5);
+  EV(6);
+  KLDI_CUDA(cudaMemcpyAsync(P->h_E, P->d_E, sizeof(double), cudaMemcpyDeviceToHost, P->stream));
+  P->have_timings = true;
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));
+  if (Exc) *Exc = *P->h_E;
+  return KLDI_OK;
+}
+
 kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
   if (!P || (option != KLDI_OPT_DETERMINISTIC_V && option != KLDI_OPT_PAIR_TEST)) {
     set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);

@@ -109,12 +109,17 @@ __device__ __forceinline__ void rho_epi_smem(const double (&acc)[16][2], double&
 
 // GGA epilogue stage: column groups J0, J0+1 of the finished X tile against the staged Phi, dxPhi, dyPhi, dzPhi
 // columns ([array][16 columns][LD]); es points at column 2 r4, row 8 warp + q4 of array 0.
+// xg (optional): global X store of the nuclear-gradient path, at (column 2 r4 of this stage, row 8 warp + q4).
 template <int J0>
 __device__ __forceinline__ void rho_epi_gga(const double (&acc)[16][2], double (&rs)[4], const double* __restrict__ es,
-                                            int eb) {
+                                            int eb, double* __restrict__ xg) {
 #pragma unroll
   for (int jj = 0; jj < 2; ++jj) {
     if (jj < eb) {
+      if (xg) {
+        xg[(jj * 8) * GB] = acc[J0 + jj][0];
+        xg[(jj * 8 + 1) * GB] = acc[J0 + jj][1];
+      }
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
         const double* e = es + (a * rho::EC + jj * 8) * LD;
@@ -141,7 +146,8 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
           const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
           const double* __restrict__ dphi2, const double* __restrict__ Dp, int n_ao, double* __restrict__ rho_s,
-          double* __restrict__ drho_s, int64_t n_pad, const unsigned long long* __restrict__ pmask) {
+          double* __restrict__ drho_s, int64_t n_pad, const unsigned long long* __restrict__ pmask,
+          double* __restrict__ x_store) {
   using namespace rho;
   extern __shared__ __align__(128) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
@@ -288,8 +294,11 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
     if (GGA && (fl & F_EPI)) {
       if constexpr (GGA) {
         const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2)
+        double* xg = nullptr;
+        if (x_store)
+          xg = x_store + (panel_off[p] + hdr[4 * s + 1] + EC * (h3 & 0xff) + 2 * r4) * GB + 8 * warp + q4;
         switch (h3 & 0xff) {
-#define KLDI_CASE(E) case E: rho_epi_gga<2 * E>(acc, rs, es, eb); break;
+#define KLDI_CASE(E) case E: rho_epi_gga<2 * E>(acc, rs, es, eb, xg); break;
           KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7)
 #undef KLDI_CASE
           default: break;
@@ -405,6 +414,58 @@ __global__ void __launch_bounds__(1024) k_sum_partials(const double* __restrict_
   if (threadIdx.x == 0) out[0] = red[0];
 }
 
+// ===================================================================================== nuclear gradient
+// dE_xc/dA_c = -2 sum_g wv_g sum_{mu on A} d_c Phi_{g,mu} X_{g,mu} (LDA, fixed grid, G1):
+// one CTA per grid block, one warp per retained column; X comes from the store the rho kernel wrote.  HBM-bound
+// (X and the three gradient stores are read once).
+__global__ void __launch_bounds__(256) k_grad_cols(const int32_t* __restrict__ tasks, const int32_t* __restrict__ kp,
+                                                   const int64_t* __restrict__ panel_off,
+                                                   const int32_t* __restrict__ colidx,
+                                                   const int32_t* __restrict__ ao_atom_c, const double* __restrict__ x,
+                                                   const double* __restrict__ d0, const double* __restrict__ d1,
+                                                   const double* __restrict__ d2, const double* __restrict__ wv_s,
+                                                   double* __restrict__ grad) {
+  const int p = tasks[blockIdx.x], lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int K = kp[p];
+  const int64_t base = panel_off[p];
+  double w[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) w[i] = wv_s[(int64_t)p * GB + 4 * lane + i];
+  for (int k = warp; k < K; k += 8) {
+    const int64_t o = (base + k) * GB + 4 * lane;
+    double t[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const double2 xv = *reinterpret_cast<const double2*>(x + o + 2 * h);
+      const double2 a = *reinterpret_cast<const double2*>(d0 + o + 2 * h);
+      const double2 b = *reinterpret_cast<const double2*>(d1 + o + 2 * h);
+      const double2 c = *reinterpret_cast<const double2*>(d2 + o + 2 * h);
+      const double x0 = w[2 * h] * xv.x, x1 = w[2 * h + 1] * xv.y;
+      t[0] += x0 * a.x + x1 * a.y;
+      t[1] += x0 * b.x + x1 * b.y;
+      t[2] += x0 * c.x + x1 * c.y;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+      for (int m = 16; m > 0; m >>= 1) t[c] += __shfl_xor_sync(0xffffffffu, t[c], m);
+    }
+    if (lane < 3) {
+      const int atom = ao_atom_c[colidx[base + k]];
+      atomicAdd(grad + 3 * atom + lane, -2.0 * (lane == 0 ? t[0] : lane == 1 ? t[1] : t[2]));
+    }
+  }
+}
+
+kldi_status launch_grad_cols(kldi_plan* P, double* grad) {
+  KLDI_CUDA(cudaMemsetAsync(grad, 0, sizeof(double) * 3 * P->n_atoms, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  k_grad_cols<<<P->n_tasks, 256, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_colidx, P->d_ao_atom_c,
+                                                 P->d_x, P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_wv_s, grad);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
 // ===================================================================================== permutations
 __global__ void k_unpermute_rho(const int32_t* __restrict__ perm, int64_t n_pad, int64_t n_pts,
                                 const double* __restrict__ rho_s, const double* __restrict__ drho_s,
@@ -462,7 +523,7 @@ kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
   return KLDI_OK;
 }
 
-kldi_status launch_rho(kldi_plan* P, bool gga) {
+kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
   kldi_status rc = set_attrs();
   if (rc != KLDI_OK) return rc;
   KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
@@ -479,12 +540,12 @@ kldi_status launch_rho(kldi_plan* P, bool gga) {
     k_rho<true, false><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
-                                                           P->n_pad, pm);
+                                                           P->n_pad, pm, x_store);
   else
     k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
                                                             nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad,
-                                                            pm);
+                                                            pm, nullptr);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }

@@ -61,6 +61,7 @@ struct kldi_plan {
   double *d_prim_alpha = nullptr, *d_prim_cn = nullptr;
   int32_t *d_shell_perm = nullptr, *d_ao_perm = nullptr;  // plan index -> caller index
   int32_t* d_ao_atom = nullptr;                           // plan AO -> plan atom rank
+  int32_t* d_ao_atom_c = nullptr;                         // plan AO -> caller atom index (nuclear gradient)
 
   // ---- grid (device), Morton order, SoA, padded to n_pad = n_blocks*128
   double *d_gx = nullptr, *d_gy = nullptr, *d_gz = nullptr, *d_gw = nullptr;
@@ -79,6 +80,7 @@ struct kldi_plan {
   double* d_dphi[3] = {nullptr, nullptr, nullptr};
   double* d_phi_v = nullptr;       // second copy of Phi in the V layout (vlayout_off)
   double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, V layout
+  double* d_x = nullptr;           // nuclear gradient: X = Phi D of every panel, rho layout, allocated on first use
 
   // ---- V contraction schedule (vsched.h), index 0: LDA upper triangle, 1: GGA square
   int32_t* d_vsched_ptr[2] = {nullptr, nullptr};  // [max_nb + 2] first pass of an nb-block panel
@@ -125,7 +127,8 @@ void plan_free(kldi_plan* P);
 kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
 // pairsel.cu
 kldi_status launch_pair_select(kldi_plan* P, bool tri);
-kldi_status launch_rho(kldi_plan* P, bool gga);
+kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store = nullptr);
+kldi_status launch_grad_cols(kldi_plan* P, double* grad);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);
 kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga);

@@ -205,7 +205,7 @@ void plan_free(kldi_plan* P) {
   if (!P) return;
   cudaSetDevice(P->device);
   void* ptrs[] = {P->d_atom_xyz, P->d_sh_atom, P->d_sh_l, P->d_sh_prim0, P->d_sh_ao0, P->d_prim_alpha, P->d_prim_cn,
-                  P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
+                  P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_ao_atom_c, P->d_x, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
                   P->d_keys, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_col_ptr, P->d_row_idx, P->d_pos,
                   P->d_blk_amax, P->d_panel_off, P->d_kp, P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                   P->d_dphi[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
@@ -263,7 +263,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   const int n_ao = P->n_ao;
 
   std::vector<double> h_axyz(3 * (size_t)n_atoms), h_alpha, h_cn;
-  std::vector<int32_t> h_sh_atom, h_sh_l, h_sh_prim0{0}, h_sh_ao0{0}, h_atom_sh0{0}, h_ao_atom;
+  std::vector<int32_t> h_sh_atom, h_sh_l, h_sh_prim0{0}, h_sh_ao0{0}, h_atom_sh0{0}, h_ao_atom, h_ao_atom_c;
   P->h_shell_perm.clear();
   P->h_ao_perm.clear();
   for (int r = 0; r < n_atoms; ++r) {
@@ -287,6 +287,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
       for (int c = 0; c < nc; ++c) {
         P->h_ao_perm.push_back(caller_ao0[s] + c);
         h_ao_atom.push_back(r);
+        h_ao_atom_c.push_back(a);
       }
       h_sh_ao0.push_back((int32_t)P->h_ao_perm.size());
     }
@@ -308,6 +309,7 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   UP(P->d_shell_perm, P->h_shell_perm);
   UP(P->d_ao_perm, P->h_ao_perm);
   UP(P->d_ao_atom, h_ao_atom);
+  UP(P->d_ao_atom_c, h_ao_atom_c);
   UP(d_atom_sh0, h_atom_sh0);
   ShellTable T{P->d_atom_xyz, P->d_sh_atom, P->d_sh_l, P->d_sh_prim0, P->d_sh_ao0, P->d_prim_alpha, P->d_prim_cn};
 

@@ -401,3 +401,35 @@ def test_full_size_sampled_parity(K, name):
     E, Vx = plan.exc(D, K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER)
     assert np.isfinite(E) and E < 0.0 and bool(torch.isfinite(Vx).all())
     plan.close()
+
+
+TOL_GRAD = 1e-9   # same bar as rho and V: a dropped block changes a gradient element by < eps * |wv X| summed like V's
+
+
+@pytest.mark.parametrize("name,n", [("cfg0", None), ("cfg1", 8), ("cfg2", 6), ("cfg4", 6)])
+def test_nuclear_gradient_parity(K, name, n):
+    """kldi_exc_grad (LDA, fixed grid) against the oracle's chain-rule contraction, element by
+    element; E_xc of the same call against the oracle energy; errors for what is not built."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional="lda")
+    plan = K.Plan.from_workload(wl, want_gradients=True)
+    D = torch.as_tensor(wl.D, device="cuda")
+    E, g = plan.exc_grad(D)
+    ref = O.exc_nuclear_gradient_lda(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D)
+    Eref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda", want_v=False)["E"]
+    g = g.cpu().numpy()
+    assert g.shape == ref.shape == (wl.n_atoms, 3)
+    assert np.max(np.abs(ref)) > 1e-3
+    assert np.max(np.abs(g - ref)) <= TOL_GRAD, np.max(np.abs(g - ref))
+    assert abs(E - Eref) <= TOL_E
+    # the same plan still serves the energy / potential path afterwards (the X store is an extra buffer)
+    E2, _ = plan.exc(D, K.KLDI_LDA_SLATER)
+    assert abs(E2 - Eref) <= TOL_E
+    with pytest.raises(K.KldiError):
+        plan.exc_grad(D, K.KLDI_GGA_PBEX)
+    plan.close()
+    plan_lda = K.Plan.from_workload(wl, want_gradients=False)
+    with pytest.raises(K.KldiError):
+        plan_lda.exc_grad(D)
+    plan_lda.close()
