@@ -155,8 +155,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pair-test", type=int, default=0, choices=[0, 1],
                     help="1: executable-pair selection a_pq*b_qr >= eps per call (Eq. 17-19)")
-    ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1],
-                    help="1: V without FP64 atomics (workspace partials + fixed-order reduce)")
+    ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1, 2],
+                    help="V without FP64 atomics: 1 = workspace partials + fixed-order reduce, 2 = fixed-point integer atomics")
+    ap.add_argument("--grad", action="store_true",
+                    help="also time kldi_exc_grad (LDA nuclear-gradient contraction) on a plan with gradient stores")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "kldi" else args.warmup
 
@@ -248,6 +250,54 @@ def main():
         e2e = {"value": 1.0 / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nn, "d2h_bytes_per_step": nn + 8,
                "ms_per_step": e2e_s * 1e3}
 
+    # ---- the same step with the bitwise-reproducible V accumulation (64-bit fixed-point integer atomics)
+    fx_leg = None
+    if world == 1 and args.deterministic_v == 0:
+        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 2)
+        for _ in range(3):
+            plan.exc(D, func, out=V)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(args.steps):
+            plan.exc(D, func, out=V)
+        f1.record()
+        torch.cuda.synchronize()
+        Va = V.clone()
+        plan.exc(D, func, out=V)
+        fx_leg = {"mode": "KLDI_OPT_DETERMINISTIC_V=2 (fixed-point integer atomics, no FP64 atomics)",
+                  "evals_per_s": 1e3 * args.steps / f0.elapsed_time(f1), "vxc_ms": plan.last_timings()["vxc"],
+                  "bitwise_equal_between_calls": bool(torch.equal(Va, V))}
+        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 0)
+
+    # ---- the LDA nuclear-gradient contraction on the same molecule (its own plan: Phi + grad Phi)
+    grad_leg = None
+    if args.grad and world == 1:
+        plan_g = K.Plan.from_workload(wl, want_gradients=True)
+        for _ in range(3):
+            plan_g.exc_grad(D)
+        tg = {}
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        g0.record()
+        for _ in range(args.steps):
+            plan_g.exc_grad(D)
+            for k, v in plan_g.last_timings().items():
+                tg[k] = tg.get(k, 0.0) + v / args.steps
+        g1.record()
+        torch.cuda.synchronize()
+        gms = g0.elapsed_time(g1) / args.steps
+        sg = plan_g.stats.as_dict()
+        col_bytes = 4 * 8 * 128 * sg["sum_k"]           # X + three gradient stores, read once by k_grad_cols
+        grad_leg = {"evals_per_s": 1e3 / gms, "ms_per_call": gms, "functional": "lda_slater",
+                    "stage_ms": {"permute_D": tg["permute_D"], "x_and_rho_build": tg["rho"], "xc": tg["xc"],
+                                 "grad_contraction": tg["vxc"]},
+                    "x_build_tflops_issued": sg["flops_rho_exec"] / (tg["rho"] * 1e-3) / 1e12,
+                    "grad_contraction_gbs": col_bytes / (tg["vxc"] * 1e-3) / 1e9,
+                    "grad_contraction_frac_of_hbm": col_bytes / (tg["vxc"] * 1e-3) / 1e9 / peaks().get("hbm_gbs", 6650.0),
+                    "sum_k": sg["sum_k"], "plan_create_s": sg["plan_seconds"]}
+        plan_g.close()
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -311,7 +361,8 @@ def main():
                                      "max_k", "phi_bytes")},
         "pair_test": {"enabled": bool(args.pair_test), "stages_total": plan.refresh_stats().pair_stages_total,
                       "stages_executed": plan.stats.pair_stages_executed},
-        "gpu_launches": 6 + (1 if gga else 0) + args.deterministic_v + 2 * args.pair_test, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+        "gpu_launches": 6 + (1 if gga else 0) + {0: 0, 1: 1, 2: 2}[args.deterministic_v] + 2 * args.pair_test, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+        "nuclear_gradient": grad_leg, "reproducible_v": fx_leg,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)

@@ -180,7 +180,11 @@ kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, d
  * KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram tile into V with
  * red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a workspace (allocated on
  * first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed order: no FP64 atomics, V bitwise
- * reproducible.
+ * reproducible; 2 = as 0, but every contribution is added as a 64-bit fixed-point integer
+ * (red.global.add.u64): integer addition is associative, so V is bitwise reproducible at the speed of mode 0.  The
+ * scale is the power of two that keeps every partial sum below 2^61, from a per-call bound
+ * max_q sum_p (sum_{g in p} |wv_g|) a_pq^2 >= |V_ij| (Eq. 11 block maxima a_pq; Cauchy-Schwarz); a contribution is
+ * rounded once, to 2^-61 of that bound, and the sum itself is exact.  Other values -> KLDI_EINVAL.
  * KLDI_OPT_PAIR_TEST: 0 (default) = the rho contraction executes every retained pair (E = I, the conservative
  * superset); 1 = per call, b_qr = max|D_qr| is formed for every AO-shell pair and a (32-column K chunk, N tile)
  * stage of the rho kernel runs only if it contains a pair with a_pq * b_qr >= eps (Eq. 17-19, t_d = eps); costs

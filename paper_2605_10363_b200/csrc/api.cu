@@ -316,7 +316,13 @@ kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
     set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);
     return KLDI_EINVAL;
   }
-  if (option == KLDI_OPT_DETERMINISTIC_V) P->v_mode = value ? 1 : 0;
+  if (option == KLDI_OPT_DETERMINISTIC_V) {
+    if (value < 0 || value > 2) {
+      set_error("kldi_plan_set_option: KLDI_OPT_DETERMINISTIC_V takes 0, 1 or 2");
+      return KLDI_EINVAL;
+    }
+    P->v_mode = value;
+  }
   if (option == KLDI_OPT_PAIR_TEST) {
     P->pair_test = value ? 1 : 0;
     if (!value) P->pair_counts_valid = false;

@@ -490,16 +490,21 @@ __global__ void k_gather_wv(const int32_t* __restrict__ perm, int64_t n_pad, int
 // H4 (V contraction) lives in vgram.cu.
 
 // ===================================================================================== H5
-template <bool GGA>
+// FIXED: Vp holds 64-bit fixed-point sums (k_vgram EPI = 2); back to double with the exact power-of-two scale.
+template <bool GGA, bool FIXED>
 __global__ void k_finalise_V(const double* __restrict__ Vp, const int32_t* __restrict__ ao_perm, int n,
-                             double* __restrict__ V) {
+                             double* __restrict__ V, const double* __restrict__ fx_bound) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= n) return;
+  const double inv = FIXED ? 1.0 / fx_scale(*fx_bound) : 1.0;
+  auto ld = [&](int64_t o) {
+    return FIXED ? (double)__double_as_longlong(Vp[o]) * inv : Vp[o];
+  };
   double v;
   if (GGA)
-    v = Vp[(int64_t)i * n + j] + Vp[(int64_t)j * n + i];  // V = B + B^T (commutative: exactly symmetric)
+    v = ld((int64_t)i * n + j) + ld((int64_t)j * n + i);  // V = B + B^T (commutative: exactly symmetric)
   else
-    v = (i <= j) ? Vp[(int64_t)i * n + j] : Vp[(int64_t)j * n + i];
+    v = (i <= j) ? ld((int64_t)i * n + j) : ld((int64_t)j * n + i);
   V[(int64_t)ao_perm[i] * n + ao_perm[j]] = v;
 }
 
@@ -578,10 +583,15 @@ kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga) {
 
 kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V) {
   dim3 grid((P->n_ao + 255) / 256, P->n_ao);
-  if (gga)
-    k_finalise_V<true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V);
+  const bool fx = P->v_mode == 2 && P->n_tasks > 0;
+  if (gga && fx)
+    k_finalise_V<true, true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, P->d_fx);
+  else if (gga)
+    k_finalise_V<true, false><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, nullptr);
+  else if (fx)
+    k_finalise_V<false, true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, P->d_fx);
   else
-    k_finalise_V<false><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V);
+    k_finalise_V<false, false><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, nullptr);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }

@@ -24,6 +24,12 @@ __host__ __device__ __forceinline__ int64_t vlayout_off(int64_t panel_off_p, int
   return panel_off_p * GB + (int64_t)rc * K8 * V_SLAB + (int64_t)col * V_SLAB + (((c ^ (col & 7)) << 1) | (rr & 1));
 }
 
+// Fixed-point scale of the V accumulation: the power of two that maps |x| <= bound below 2^61.
+__host__ __device__ __forceinline__ double fx_scale(double bound) {
+  if (!(bound > 0.0)) return 1.0;
+  return scalbn(1.0, 60 - ilogb(bound));
+}
+
 #define KLDI_CUDA(call)                                                                     \
   do {                                                                                      \
     cudaError_t e__ = (call);                                                               \
@@ -91,7 +97,9 @@ struct kldi_plan {
   double* d_gram = nullptr;                       // lazily allocated workspace of G_p partials
   int64_t gram_cap = 0;
   int32_t* d_ao_shell = nullptr;                  // plan AO -> plan shell
-  int v_mode = 0;                                 // 0: red.global.add epilogue, 1: workspace + fixed-order reduce
+  int v_mode = 0;                                 // 0: red.global.add.f64 epilogue, 1: workspace + fixed-order reduce,
+                                                  // 2: 64-bit fixed-point integer atomics (reproducible)
+  double* d_fx = nullptr;                         // [1 + n_blocks] fixed-point bound, then s_p = sum_g |wv_g| per block
   // ---- executable-pair selection (pairsel.cu), allocated on first use
   int pair_test = 0;
   double* d_bmax = nullptr;                       // [n_shells][n_shells] b_qr = max|D_qr|

@@ -64,16 +64,21 @@ __device__ __forceinline__ void vg_run(double (&acc)[2][4][2], const double* __r
   }
 }
 
-// ATOMIC = true : the epilogue adds G_p straight into the plan-order V with red.global.add.f64.
-// ATOMIC = false: G_p goes to the workspace (plain 16-B stores) and k_vreduce sums it in a fixed order.
-template <bool GGA, bool ATOMIC>
+// EPI = 0: the epilogue adds G_p straight into the plan-order V with red.global.add.f64.
+// EPI = 1: G_p goes to the workspace (plain 16-B stores) and k_vreduce sums it in a fixed order.
+// EPI = 2: as 0, but in 64-bit fixed point with integer atomics: integer addition is associative, so V is bitwise
+//          reproducible whatever the order of the adds; the scale is the power of two that keeps every partial sum
+//          below 2^61 (k_fx_bound), the only rounding is that of a contribution to 2^-61 of the bound.
+template <bool GGA, int EPI>
 __global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
     k_vgram(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
             const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
             const double* __restrict__ phi, const double* __restrict__ zmat, const double* __restrict__ wv_s,
             const int32_t* __restrict__ sched_ptr, const VPass* __restrict__ passes, const VItem* __restrict__ items,
-            int n_ao, double* __restrict__ Vp, const int64_t* __restrict__ gram_off, double* __restrict__ G) {
+            int n_ao, double* __restrict__ Vp, const int64_t* __restrict__ gram_off, double* __restrict__ G,
+            const double* __restrict__ fx_bound) {
   using namespace vg;
+  constexpr bool ATOMIC = (EPI != 1);
   extern __shared__ __align__(128) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
   const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);  // full[s] at +8s, empty[s] at +8(NST+s)
@@ -145,6 +150,7 @@ __global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
   const int q4 = lane >> 2, r4 = lane & 3;
   const int o0 = ((2 * r4) ^ q4) * 2, o1 = ((2 * r4 + 1) ^ q4) * 2;  // swizzled chunk offsets (doubles)
   double acc[V_SLOTS][2][4][2];
+  const double fxs = (EPI == 2) ? fx_scale(*fx_bound) : 1.0;
   int ia[V_SLOTS], ib[V_SLOTS];
 #pragma unroll
   for (int k = 0; k < V_SLOTS; ++k) ia[k] = ib[k] = 0;
@@ -210,7 +216,13 @@ __global__ void __launch_bounds__(32 * (V_WARPS + 1), 1)
 #pragma unroll
                   for (int e = 0; e < 2; ++e) {
                     const int c = bcol + 8 * j + 2 * r4 + e;
-                    if (c < K && (GGA || r <= c)) atomicAdd(Vp + ci + cidx[8 * j + e], acc[k][mi][j][e]);
+                    if (c < K && (GGA || r <= c)) {
+                      if (EPI == 2)
+                        atomicAdd(reinterpret_cast<unsigned long long*>(Vp) + ci + cidx[8 * j + e],
+                                  (unsigned long long)__double2ll_rn(acc[k][mi][j][e] * fxs));
+                      else
+                        atomicAdd(Vp + ci + cidx[8 * j + e], acc[k][mi][j][e]);
+                    }
                   }
                 }
             }
@@ -313,19 +325,71 @@ __global__ void __launch_bounds__(128) k_build_z(const int32_t* __restrict__ kp,
   }
 }
 
-template <bool GGA, bool ATOMIC>
+// Fixed-point mode (EPI = 2): a bound on every partial sum of every V entry.  |G_p[i,j]| <= s_p a_pi a_pj with
+// s_p = sum_{g in p} |wv_g| (GGA: 1/2|wv_0| + |wv_1| + |wv_2| + |wv_3|, the weights of Z) and a_pq the block maxima
+// of the filter (Eq. 11), so by Cauchy-Schwarz |sum_p G_p[i,j]| <= sqrt(b_i b_j) <= max_q b_q,
+// b_q = sum_{p in BCS(C) column q} s_p a_pq^2.  Fixed reduction trees and an associative max: the bound, and with it
+// V, is reproducible.
+__global__ void __launch_bounds__(256) k_fx_block_sums(int64_t n_blocks, int64_t n_pad, int ncomp,
+                                                       const double* __restrict__ wv_s, double* __restrict__ s_p) {
+  const int64_t p = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (p >= n_blocks) return;
+  double a = 0.0;
+  for (int c = 0; c < ncomp; ++c) {
+    double t = 0.0;
+    for (int i = 0; i < 4; ++i) t += fabs(wv_s[c * n_pad + p * GB + lane + 32 * i]);
+    a += (ncomp == 4 && c == 0) ? 0.5 * t : t;
+  }
+  for (int m = 16; m > 0; m >>= 1) a += __shfl_xor_sync(0xffffffffu, a, m);
+  if (lane == 0) s_p[p] = a;
+}
+// one CTA per AO shell (a BCS(C) column can hold thousands of grid blocks)
+__global__ void __launch_bounds__(256) k_fx_bound(const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ row_idx,
+                                                  const int32_t* __restrict__ pos, const double* __restrict__ amax,
+                                                  const double* __restrict__ s_p, double* __restrict__ bound) {
+  __shared__ double red[8];
+  const int q = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double b = 0.0;
+  for (int e = col_ptr[q] + threadIdx.x; e < col_ptr[q + 1]; e += 256) {
+    const double a = amax[pos[e]];
+    b += s_p[row_idx[e]] * a * a;
+  }
+  for (int m = 16; m > 0; m >>= 1) b += __shfl_xor_sync(0xffffffffu, b, m);
+  if (lane == 0) red[warp] = b;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) b += red[w];
+    // b >= 0: the bit pattern of a non-negative double orders like the value
+    atomicMax(reinterpret_cast<unsigned long long*>(bound), (unsigned long long)__double_as_longlong(b));
+  }
+}
+
+static kldi_status launch_fx_bound(kldi_plan* P, bool gga) {
+  if (!P->d_fx) KLDI_CUDA(cudaMalloc(&P->d_fx, sizeof(double) * (size_t)(P->n_blocks + 1)));
+  KLDI_CUDA(cudaMemsetAsync(P->d_fx, 0, sizeof(double), P->stream));
+  k_fx_block_sums<<<(int)((P->n_blocks + 7) / 8), 256, 0, P->stream>>>(P->n_blocks, P->n_pad, gga ? 4 : 1, P->d_wv_s,
+                                                                      P->d_fx + 1);
+  KLDI_CUDA(cudaGetLastError());
+  k_fx_bound<<<P->n_shells, 256, 0, P->stream>>>(P->d_col_ptr, P->d_row_idx, P->d_pos, P->d_blk_amax, P->d_fx + 1,
+                                                 P->d_fx);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+template <bool GGA, int EPI>
 static kldi_status launch_vgram(kldi_plan* P) {
   static bool attr_done = false;
   if (!attr_done) {
-    KLDI_CUDA(cudaFuncSetAttribute(k_vgram<GGA, ATOMIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, vg::SMEM_BYTES));
+    KLDI_CUDA(cudaFuncSetAttribute(k_vgram<GGA, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, vg::SMEM_BYTES));
     attr_done = true;
   }
   const int m = GGA ? 1 : 0;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
-  k_vgram<GGA, ATOMIC><<<grid, 32 * (V_WARPS + 1), vg::SMEM_BYTES, P->stream>>>(
+  k_vgram<GGA, EPI><<<grid, 32 * (V_WARPS + 1), vg::SMEM_BYTES, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi_v, P->d_z, P->d_wv_s,
       P->d_vsched_ptr[m], static_cast<const VPass*>(P->d_vpasses[m]), static_cast<const VItem*>(P->d_vitems[m]),
-      P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram);
+      P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram, P->d_fx);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }
@@ -429,9 +493,9 @@ static kldi_status launch_vreduce(kldi_plan* P) {
 
 kldi_status launch_vxc(kldi_plan* P, bool gga) {
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
-  if (P->v_mode == 0) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+  if (P->v_mode != 1) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
   if (P->n_tasks == 0) {
-    if (P->v_mode != 0) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+    if (P->v_mode == 1) KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
     return KLDI_OK;
   }
   if (gga) {
@@ -439,7 +503,12 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
                                                        P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_z);
     KLDI_CUDA(cudaGetLastError());
   }
-  if (P->v_mode == 0) return gga ? launch_vgram<true, true>(P) : launch_vgram<false, true>(P);
+  if (P->v_mode == 0) return gga ? launch_vgram<true, 0>(P) : launch_vgram<false, 0>(P);
+  if (P->v_mode == 2) {
+    kldi_status rc = launch_fx_bound(P, gga);
+    if (rc != KLDI_OK) return rc;
+    return gga ? launch_vgram<true, 2>(P) : launch_vgram<false, 2>(P);
+  }
   // deterministic mode: G_p partials to the workspace, then the fixed-order reduce
   const int m = gga ? 1 : 0;
   if (P->gram_cap < P->gram_elems[m]) {
@@ -449,7 +518,7 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
     KLDI_CUDA(cudaMalloc(&P->d_gram, sizeof(double) * (size_t)std::max<int64_t>(1, P->gram_elems[m])));
     P->gram_cap = P->gram_elems[m];
   }
-  kldi_status rc = gga ? launch_vgram<true, false>(P) : launch_vgram<false, false>(P);
+  kldi_status rc = gga ? launch_vgram<true, 1>(P) : launch_vgram<false, 1>(P);
   if (rc != KLDI_OK) return rc;
   return gga ? launch_vreduce<true>(P) : launch_vreduce<false>(P);
 }

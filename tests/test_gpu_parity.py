@@ -303,14 +303,15 @@ def test_reproducible_rho_and_energy(K):
     plan.close()
 
 
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("name,n,fn", [("cfg1", 8, "lda"), ("cfg4", 6, "gga"), ("cfg0", None, "lda")])
-def test_deterministic_v_mode(K, name, n, fn):
-    """KLDI_OPT_DETERMINISTIC_V: Gram partials in a workspace + fixed-order reduce (no FP64 atomics):
-    same parity bar, and V bitwise identical between calls."""
+def test_deterministic_v_mode(K, name, n, fn, mode):
+    """KLDI_OPT_DETERMINISTIC_V = 1: Gram partials in a workspace + fixed-order reduce; = 2: 64-bit fixed-point
+    integer atomics (associative).  Neither uses FP64 atomics: same parity bar, and V bitwise identical between calls."""
     import torch
 
     wl = W.named_config(name, n_override=n, functional=fn)
-    out = run_gpu(K, wl, deterministic_v=1)
+    out = run_gpu(K, wl, deterministic_v=mode)
     ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, fn)
     check(out, ref)
     plan = out["plan"]
