@@ -327,6 +327,9 @@ def main():
             "flops_per_launch": f_rho, "exec_flops_per_launch": f_rho_exec,
             "exec_frac": f_rho_exec / t_rho / 1e12 / fp64_clock_peak,
             "launch_ms": stage_ms["rho"], "traffic": None,
+            # DMMA.8x8x4 itself tops out below the FP64 unit rate (profiles/r1f_summary.md): issued FLOPs against it
+            "dmma_instruction_cap_tflops": dmma_live,
+            "exec_frac_of_dmma_cap": (f_rho_exec / t_rho / 1e12 / dmma_live) if dmma_live else None,
             "v_kernel": {"achieved": f_v / (stage_ms["vxc"] * 1e-3) / 1e12, "launch_ms": stage_ms["vxc"],
                          "frac": f_v / (stage_ms["vxc"] * 1e-3) / 1e12 / fp64_clock_peak,
                          "flops_per_launch": f_v, "exec_flops_per_launch": st["flops_v_exec"],
