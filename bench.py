@@ -247,7 +247,10 @@ def main():
         torch.cuda.synchronize()
         e2e_s = (time.perf_counter() - t0) / args.steps
         nn = wl.n_ao * wl.n_ao * 8
-        e2e = {"value": 1.0 / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nn, "d2h_bytes_per_step": nn + 8,
+        bands = 1 if wl.n_ao < 1024 else 32           # kldi_exc_host uploads the lower triangle of D in row bands
+        h2d = sum(8 * (wl.n_ao * (b + 1) // bands) * (wl.n_ao * (b + 1) // bands - wl.n_ao * b // bands)
+                  for b in range(bands))
+        e2e = {"value": 1.0 / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": nn + 8,
                "ms_per_step": e2e_s * 1e3}
 
     # ---- the same step with the bitwise-reproducible V accumulation (64-bit fixed-point integer atomics)

@@ -132,7 +132,8 @@ kldi_status kldi_build_vxc(kldi_plan* plan, const double* wv, int gga, double* V
 kldi_status kldi_exc(kldi_plan* plan, const double* D, kldi_functional f, double* Exc, double* V);
 
 /* Same as kldi_exc with HOST buffers: copies D to the device, runs, copies V back (end-to-end
- * timing; D_host/V_host should be page-locked for full PCIe speed but need not be). */
+ * timing; D_host/V_host should be page-locked for full PCIe speed but need not be).  D is symmetric and only its
+ * lower triangle (row >= column) is read, here and in every other call: kldi_exc_host uploads just that half. */
 kldi_status kldi_exc_host(kldi_plan* plan, const double* D_host, kldi_functional f, double* Exc,
                           double* V_host);
 

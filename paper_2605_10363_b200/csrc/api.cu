@@ -268,7 +268,18 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
   if (!P->d_stage_host) KLDI_CUDA(cudaMalloc(&P->d_stage_host, 2 * nn));
   double* dD = P->d_stage_host;
   double* dV = V_host ? P->d_stage_host + (size_t)P->n_ao * P->n_ao : nullptr;
-  KLDI_CUDA(cudaMemcpyAsync(dD, D_host, nn, cudaMemcpyHostToDevice, P->stream));
+  // D is symmetric and k_permute_D reads only its lower triangle: upload that half, in 32 row bands (band [r0, r1)
+  // needs the columns [0, r1)), 52 % of the bytes of the full matrix over PCIe
+  {
+    const int n = P->n_ao, nb = n < 1024 ? 1 : 32;
+    for (int b = 0; b < nb; ++b) {
+      const int r0 = (int)((int64_t)n * b / nb), r1 = (int)((int64_t)n * (b + 1) / nb);
+      if (r1 > r0)
+        KLDI_CUDA(cudaMemcpy2DAsync(dD + (size_t)r0 * n, sizeof(double) * n, D_host + (size_t)r0 * n,
+                                    sizeof(double) * n, sizeof(double) * r1, r1 - r0, cudaMemcpyHostToDevice,
+                                    P->stream));
+    }
+  }
   kldi_status rc = exc_enqueue(P, dD, f, dV);
   if (rc != KLDI_OK) return rc;
   if (V_host) KLDI_CUDA(cudaMemcpyAsync(V_host, dV, nn, cudaMemcpyDeviceToHost, P->stream));

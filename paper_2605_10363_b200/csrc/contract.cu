@@ -28,7 +28,9 @@ __global__ void k_permute_D(const double* __restrict__ D, const int32_t* __restr
   if (j >= n) return;
   double v = 0.0;
   if (!TRI || j <= i) {
-    v = D[(int64_t)ao_perm[i] * n + ao_perm[j]];
+    // D is symmetric (kldi.h): always read its lower triangle, so that kldi_exc_host only has to upload that half
+    const int a = ao_perm[i], b = ao_perm[j];
+    v = D[(int64_t)max(a, b) * n + min(a, b)];
     if (TRI && j == i) v *= 0.5;
   }
   Dp[(int64_t)i * n + j] = v;

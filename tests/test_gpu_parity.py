@@ -434,3 +434,26 @@ def test_nuclear_gradient_parity(K, name, n):
     with pytest.raises(K.KldiError):
         plan_lda.exc_grad(D)
     plan_lda.close()
+
+
+@pytest.mark.parametrize("n", [4, 44])
+def test_exc_host_equals_device_path_and_reads_lower_triangle_only(K, n):
+    """kldi_exc_host (host buffers; single band below 1024 AOs, 32 row bands above): same E and V as kldi_exc, and D's
+    strict upper triangle is never read (include/kldi.h) — poisoning it with NaN changes nothing."""
+    import torch
+
+    wl = W.named_config("cfg1", n_override=n)
+    plan = K.Plan.from_workload(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 2)      # bitwise reproducible V, so the comparison can be exact
+    E0, V0 = plan.exc(D)
+    Dh = torch.as_tensor(wl.D).clone()
+    Dh[torch.triu(torch.ones_like(Dh, dtype=torch.bool), diagonal=1)] = float("nan")
+    Vh = torch.empty_like(Dh)
+    E1 = plan.exc_host(Dh.pin_memory(), K.KLDI_LDA_SLATER, Vh)
+    assert E1 == E0 and torch.equal(Vh, V0.cpu())
+    Dn = D.clone()
+    Dn[torch.triu(torch.ones_like(Dn, dtype=torch.bool), diagonal=1)] = float("nan")
+    E2, V2 = plan.exc(Dn)
+    assert E2 == E0 and torch.equal(V2, V0)
+    plan.close()
