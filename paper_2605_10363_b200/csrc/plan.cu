@@ -454,6 +454,12 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   UP(P->d_panel_off, panel_off);
   UP(P->d_kp, h_kp);
   UP(P->d_colidx, h_colidx);
+  // S: cost-sorted pull order.  Heavy grid blocks first so that the tail of the persistent kernels is made of light
+  // ones; buckets of 96 columns, Morton order kept inside a bucket for the L2 locality of the D gather (measured:
+  // cfg1 +2 %, cfg2 +1 %, cfg3 +0.3 % over plain Morton order; fully sorted by K_p loses the locality again).
+  constexpr int TASK_BUCKET = 96;
+  std::stable_sort(h_tasks.begin(), h_tasks.end(),
+                   [&](int32_t a, int32_t b) { return h_kp[a] / TASK_BUCKET > h_kp[b] / TASK_BUCKET; });
   UP(P->d_tasks, h_tasks);
   P->n_tasks = (int32_t)h_tasks.size();
   {
