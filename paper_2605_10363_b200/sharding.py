@@ -4,7 +4,7 @@ The paper distributes filtered grid batches over GPUs and reduces the partial EX
 at the end (§III-E).  Here each rank owns a contiguous range of the caller's
 grid points (whole atomic grids where possible, so a rank's points are spatially compact), builds
 its own kldi plan on that range, and the only exchange step is one all-reduce(sum) of V
-([n_ao][n_ao] FP64) and of the scalar E_xc.  rho stays sharded.  D is replicated.
+([n_ao][n_ao] FP64; or of the [n_atoms][3] nuclear gradient) and of the scalar E_xc.  rho stays sharded.  D is replicated.
 
 This module holds host logic only (index arithmetic and the torch.distributed calls); it is
 exercised on CPU with the gloo backend in tests/test_sharding.py.
@@ -37,7 +37,8 @@ def shard_workload(wl, rank: int, world_size: int, align: int = 5500):
 
 def allreduce_exc(E_local: float, V_local, group=None):
     """Sum the per-rank partial energy and potential matrix over all ranks (in place on V_local).
-    V_local: torch tensor on the backend's device (cuda for nccl, cpu for gloo)."""
+    V_local: torch tensor on the backend's device (cuda for nccl, cpu for gloo).  The nuclear gradient of
+    kldi_exc_grad is a sum over grid points too: pass the rank's [n_atoms][3] partial instead of V."""
     import torch
     import torch.distributed as dist
 

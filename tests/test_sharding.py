@@ -44,7 +44,9 @@ def _worker(rank, world, port, out_dir):
     basis = (wl.atom_xyz, wl.shell_atom, wl.shell_l, wl.shell_prim_off, wl.prim_alpha, wl.prim_coef)
     loc = O.exc(basis, part.grid_xyz, part.grid_w, part.D, "lda")
     E, V = sharding.allreduce_exc(loc["E"], torch.as_tensor(loc["V"].copy()))
-    np.savez(os.path.join(out_dir, f"r{rank}.npz"), E=E, V=V.numpy(), lo=lo, hi=hi, rho=loc["rho"])
+    g_loc = O.exc_nuclear_gradient_lda(basis, part.grid_xyz, part.grid_w, part.D)
+    _, g = sharding.allreduce_exc(loc["E"], torch.as_tensor(g_loc.copy()))
+    np.savez(os.path.join(out_dir, f"r{rank}.npz"), E=E, V=V.numpy(), lo=lo, hi=hi, rho=loc["rho"], grad=g.numpy())
     dist.destroy_process_group()
 
 
@@ -63,3 +65,6 @@ def test_two_rank_gloo_matches_single(tmp_path):
         assert abs(float(p["E"]) - ref["E"]) < 1e-12
         assert np.max(np.abs(p["V"] - ref["V"])) < 1e-12
     assert np.max(np.abs(np.concatenate([p["rho"] for p in parts]) - ref["rho"])) < 1e-13
+    gref = O.exc_nuclear_gradient_lda(basis, wl.grid_xyz, wl.grid_w, wl.D)
+    for p in parts:   # the nuclear gradient is a sum over grid shards as well
+        assert np.max(np.abs(p["grad"] - gref)) < 1e-12
