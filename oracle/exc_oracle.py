@@ -22,7 +22,8 @@ dense-product step; `brute_force_lda` below is the same thing as explicit Python
 Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): analytic Gaussian overlap => diag(S)=1 and
 int rho = Tr(D S); closed-form Slater energy of one s-Gaussian; V symmetric; central finite
 differences dE/dD = V (LDA and PBE-x); brute-force loops on single water; PBE-x limits; central finite
-differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda.
+differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda; kinetic-energy density: closed
+form int tau = 3 alpha n / 2 of one s-Gaussian, AO gradients from finite differences, Tr(D V^tau) = sum wv tau.
 Absolute PBE-x energies have no printed reference value: beyond the limits and the FD
 identity they are "parity unpinned".
 """
@@ -223,6 +224,20 @@ def exc_energy_from_rho(w, rho, drho=None, functional: str = "lda") -> float:
     else:
         e, _ = slater(rho)
     return math.fsum((np.asarray(w) * e).tolist())
+
+
+# ----------------------------------------------------------------------------- meta-GGA contractions
+def kinetic_energy_density(dphi, D):
+    """tau_g = 1/2 sum_{mu,nu} D_{mu,nu} grad chi_mu(r_g) . grad chi_nu(r_g): the third density-like variable of the
+    meta-GGA class the paper runs (M06-2X; the functional itself is out of scope).  The same product
+    as the density build (Eq. 4) with d_c Phi in place of Phi, summed over c."""
+    return 0.5 * sum(np.sum((dphi[c] @ D) * dphi[c], axis=1) for c in range(3))
+
+
+def vtau_from_wv(dphi, wv):
+    """V^tau = 1/2 sum_c (d_c Phi)^T diag(wv) (d_c Phi), wv = w * v_tau: dE/dD_{mu,nu} of E = sum_g w_g e(tau_g)
+    (Eq. 5, with d_c Phi in place of Phi)."""
+    return 0.5 * sum(dphi[c].T @ (wv[:, None] * dphi[c]) for c in range(3))
 
 
 # ----------------------------------------------------------------------------- nuclear gradient (SURVEY.md §8(f2))

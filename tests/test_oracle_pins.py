@@ -155,6 +155,44 @@ def test_nuclear_gradient_lda_matches_finite_difference_of_energy(water):
         assert abs(g[:, c].sum() + np.dot(wv, drho[c])) < 1e-10 * np.max(np.abs(g))
 
 
+def test_kinetic_energy_density_and_vtau(water):
+    """SURVEY.md §8(f4) contractions.  (a) closed form: one normalised s-Gaussian, exponent alpha, occupation n has
+    int tau = n * 3 alpha / 2 (its kinetic energy); (b) tau from AO gradients taken by central differences of the AO
+    VALUES (independent of the analytic gradients); (c) V^tau is symmetric, and Tr(D V^tau[wv]) = sum_g wv_g tau_g
+    for arbitrary wv (a wrong factor or transposed operand in either function breaks it); (d) one element by loops."""
+    from paper_2605_10363_b200 import workloads as W
+
+    alpha, n = 0.9, 2.0
+    pts, w = W.atomic_grid(1.0, n_rad=120)
+    one = (np.zeros((1, 3)), np.array([0]), np.array([0]), np.array([0, 1]), np.array([alpha]), np.array([1.0]))
+    _, dphi = O.ao_values(*one, pts, deriv=True)
+    tau = O.kinetic_energy_density(dphi, np.array([[n]]))
+    assert abs(np.dot(w, tau) - 1.5 * alpha * n) < 1e-8
+
+    basis = basis_of(water)
+    rng = np.random.default_rng(11)
+    p2 = rng.uniform(-2.0, 2.0, size=(30, 3))
+    _, dphi = O.ao_values(*basis, p2, deriv=True)
+    tau = O.kinetic_energy_density(dphi, water.D)
+    h = 1e-5
+    fd = []
+    for c in range(3):
+        e = np.zeros(3); e[c] = h
+        fd.append((O.ao_values(*basis, p2 + e) - O.ao_values(*basis, p2 - e)) / (2 * h))
+    tau_fd = 0.5 * sum(np.einsum("gm,mn,gn->g", fd[c], water.D, fd[c]) for c in range(3))
+    assert np.max(np.abs(tau - tau_fd)) < 1e-7 * np.max(np.abs(tau))
+    wv = rng.normal(size=len(p2))
+    Vt = O.vtau_from_wv(dphi, wv)
+    assert np.max(np.abs(Vt - Vt.T)) <= 1e-14 * np.max(np.abs(Vt))
+    assert abs(np.sum(water.D * Vt) - np.dot(wv, tau)) < 1e-11 * abs(np.dot(np.abs(wv), tau))
+    m, k = 3, 17
+    loop = 0.0
+    for g in range(len(p2)):
+        for c in range(3):
+            loop += 0.5 * wv[g] * dphi[c][g, m] * dphi[c][g, k]
+    assert abs(loop - Vt[m, k]) < 1e-13 * np.max(np.abs(Vt))
+
+
 def test_pbe_enhancement_limits():
     rho = np.geomspace(1e-12, 50.0, 200)
     e_s, v_s = O.slater(rho)
