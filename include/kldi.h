@@ -166,6 +166,18 @@ kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_
 kldi_status kldi_plan_export_tile(const kldi_plan* plan, int64_t entry, int c, double* out,
                                   int64_t cap_bytes, int32_t* width);
 
+/* Meta-GGA contractions (the paper's functional class, PAPER.md:270 — the functional itself is not
+ * part of the library): the density build and the V accumulation (Eq. 4 / Eq. 5) with the stored AO
+ * gradients in place of Phi, over the same retained block pairs.  Both need want_gradients = 1 (else KLDI_ESTATE).
+ *   kldi_eval_tau  : tau[g] = 1/2 sum_{mu,nu} D_{mu,nu} grad chi_mu(r_g) . grad chi_nu(r_g);  D dev [n_ao][n_ao]
+ *                    symmetric, tau dev [n_pts], caller grid order, overwritten.
+ *   kldi_build_vtau: V = 1/2 sum_c (d_c Phi)^T diag(wv_tau) (d_c Phi), wv_tau = w * v_tau dev [n_pts];  V dev
+ *                    [n_ao][n_ao], overwritten, exactly symmetric (add it to the V of kldi_build_vxc).  Accumulation
+ *                    follows KLDI_OPT_DETERMINISTIC_V (1 runs as 2).
+ * Asynchronous on the plan's stream. */
+kldi_status kldi_eval_tau(kldi_plan* plan, const double* D, double* tau);
+kldi_status kldi_build_vtau(kldi_plan* plan, const double* wv_tau, double* V);
+
 /* EXC nuclear-gradient contraction (the paper's second workload; it prints no formula, so this is
  * the chain rule on E_xc = sum_g w_g e(rho_g), DESIGN.md §3 reading G1): at fixed D and FIXED quadrature (points and
  * weights do not follow the atoms, no grid response),

@@ -20,7 +20,7 @@ KLDI_GGA_PBEX = 1
 
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
-    "kldi_exc_host", "kldi_exc_grad", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
+    "kldi_exc_host", "kldi_exc_grad", "kldi_eval_tau", "kldi_build_vtau", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
     "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
     "kldi_vlayout_offset",
 ]
@@ -82,6 +82,8 @@ def lib():
         L.kldi_exc.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_exc_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_exc_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        L.kldi_eval_tau.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.kldi_build_vtau.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.kldi_last_timings.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.kldi_plan_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_plan_export_tile.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_int64,
@@ -210,6 +212,24 @@ class Plan:
         _check(lib().kldi_exc(self._h, self._dev64(D, (self.n_ao, self.n_ao), "D"), int(functional), C.byref(e),
                               self._dev64(V, (self.n_ao, self.n_ao), "V") if want_v else None), "kldi_exc")
         return e.value, V
+
+    def eval_tau(self, D):
+        """kldi_eval_tau: the kinetic-energy density on the caller's grid order, device tensor [n_pts]."""
+        import torch
+
+        tau = torch.empty(self.n_pts, dtype=torch.float64, device=self.device)
+        _check(lib().kldi_eval_tau(self._h, self._dev64(D, (self.n_ao, self.n_ao), "D"), C.c_void_p(tau.data_ptr())),
+               "kldi_eval_tau")
+        return tau
+
+    def build_vtau(self, wv_tau, out=None):
+        """kldi_build_vtau: V = 1/2 sum_c (d_c Phi)^T diag(wv_tau) (d_c Phi)."""
+        import torch
+
+        V = out if out is not None else torch.empty((self.n_ao, self.n_ao), dtype=torch.float64, device=self.device)
+        _check(lib().kldi_build_vtau(self._h, self._dev64(wv_tau, (self.n_pts,), "wv_tau"),
+                                     self._dev64(V, (self.n_ao, self.n_ao), "V")), "kldi_build_vtau")
+        return V
 
     def exc_grad(self, D, functional: int = KLDI_LDA_SLATER):
         """kldi_exc_grad: (E_xc, grad [n_atoms][3] device tensor, caller atom order)."""

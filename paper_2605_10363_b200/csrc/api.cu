@@ -288,6 +288,52 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
   return KLDI_OK;
 }
 
+kldi_status kldi_eval_tau(kldi_plan* P, const double* D, double* tau) {
+  if (!P || !D || !tau) {
+    set_error("kldi_eval_tau: null argument");
+    return KLDI_EINVAL;
+  }
+  if (!P->want_grad) {
+    set_error("kldi_eval_tau: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
+    return KLDI_ESTATE;
+  }
+  kldi_status rc;
+  P->have_timings = false;
+  EV(0);
+  if ((rc = launch_permute_D(P, D, false)) != KLDI_OK) return rc;  // triangular D': the product is symmetric in mu, nu
+  EV(1);
+  for (int c = 0; c < 3; ++c)
+    if ((rc = launch_rho_lda_on(P, P->d_dphi[c], P->d_drho_s + (size_t)c * P->n_pad)) != KLDI_OK) return rc;
+  if ((rc = launch_tau_combine(P)) != KLDI_OK) return rc;
+  EV(2);
+  if ((rc = launch_unpermute_rho(P, tau, nullptr)) != KLDI_OK) return rc;
+  for (int i = 3; i < 7; ++i) EV(i);
+  P->have_timings = true;
+  return KLDI_OK;
+}
+
+kldi_status kldi_build_vtau(kldi_plan* P, const double* wv_tau, double* V) {
+  if (!P || !wv_tau || !V) {
+    set_error("kldi_build_vtau: null argument");
+    return KLDI_EINVAL;
+  }
+  if (!P->want_grad) {
+    set_error("kldi_build_vtau: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
+    return KLDI_ESTATE;
+  }
+  kldi_status rc;
+  P->have_timings = false;
+  for (int i = 0; i < 4; ++i) EV(i);
+  if ((rc = launch_gather_wv(P, wv_tau, false, 0.5)) != KLDI_OK) return rc;
+  EV(4);
+  if ((rc = launch_vtau(P)) != KLDI_OK) return rc;
+  EV(5);
+  if ((rc = launch_finalise_V(P, false, V, P->v_mode != 0)) != KLDI_OK) return rc;
+  EV(6);
+  P->have_timings = true;
+  return KLDI_OK;
+}
+
 kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, double* Exc, double* grad) {
   if (!P || !D || !grad) {
     set_error("kldi_exc_grad: null argument");

@@ -482,11 +482,17 @@ __global__ void k_unpermute_rho(const int32_t* __restrict__ perm, int64_t n_pad,
 }
 
 __global__ void k_gather_wv(const int32_t* __restrict__ perm, int64_t n_pad, int64_t n_pts, int ncomp,
-                            const double* __restrict__ wv, double* __restrict__ wv_s) {
+                            const double* __restrict__ wv, double* __restrict__ wv_s, double scale) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_pad) return;
   const int64_t g = perm[i];
-  for (int c = 0; c < ncomp; ++c) wv_s[c * n_pad + i] = (g >= 0) ? wv[c * n_pts + g] : 0.0;
+  for (int c = 0; c < ncomp; ++c) wv_s[c * n_pad + i] = (g >= 0) ? scale * wv[c * n_pts + g] : 0.0;
+}
+
+// tau_g = 1/2 sum_c t_c(g), t_c = sum_{mu,nu} D_{mu,nu} d_c chi_mu d_c chi_nu from three LDA-form rho builds
+__global__ void k_tau_combine(int64_t n_pad, const double* __restrict__ t, double* __restrict__ tau_s) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_pad) tau_s[i] = 0.5 * (t[i] + t[n_pad + i] + t[2 * n_pad + i]);
 }
 
 // H4 (V contraction) lives in vgram.cu.
@@ -557,6 +563,29 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
   return KLDI_OK;
 }
 
+// The LDA-form (triangular D') rho build on another store of the rho layout: out_s[g] = sum_{mu,nu} D_{mu,nu}
+// A_{g,mu} A_{g,nu} with A = d_c Phi (kinetic-energy density).  D' must already be in P->d_Dp.
+kldi_status launch_rho_lda_on(kldi_plan* P, const double* store, double* out_s) {
+  kldi_status rc = set_attrs();
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaMemsetAsync(out_s, 0, sizeof(double) * P->n_pad, P->stream));
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, store, nullptr, nullptr, nullptr,
+      P->d_Dp, P->n_ao, out_s, nullptr, P->n_pad, nullptr, nullptr);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+kldi_status launch_tau_combine(kldi_plan* P) {
+  const int nb = (int)((P->n_pad + 255) / 256);
+  k_tau_combine<<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_drho_s, P->d_rho_s);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho) {
   const int nb = (int)((P->n_pad + 255) / 256);
   k_unpermute_rho<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, P->d_rho_s, P->d_drho_s, rho, drho);
@@ -576,16 +605,16 @@ kldi_status launch_xc(kldi_plan* P, kldi_functional f) {
   return KLDI_OK;
 }
 
-kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga) {
+kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga, double scale) {
   const int nb = (int)((P->n_pad + 255) / 256);
-  k_gather_wv<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, gga ? 4 : 1, wv, P->d_wv_s);
+  k_gather_wv<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, gga ? 4 : 1, wv, P->d_wv_s, scale);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }
 
-kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V) {
+kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V, int fixed) {
   dim3 grid((P->n_ao + 255) / 256, P->n_ao);
-  const bool fx = P->v_mode == 2 && P->n_tasks > 0;
+  const bool fx = (fixed < 0 ? P->v_mode == 2 : fixed != 0) && P->n_tasks > 0;
   if (gga && fx)
     k_finalise_V<true, true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, P->d_fx);
   else if (gga)

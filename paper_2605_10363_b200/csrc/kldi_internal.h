@@ -139,9 +139,12 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store = nullptr);
 kldi_status launch_grad_cols(kldi_plan* P, double* grad);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);
-kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga);
+kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga, double scale = 1.0);
+kldi_status launch_rho_lda_on(kldi_plan* P, const double* store, double* out_s);
+kldi_status launch_tau_combine(kldi_plan* P);
+kldi_status launch_vtau(kldi_plan* P);
 kldi_status launch_vxc(kldi_plan* P, bool gga);
-kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V);
+kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V, int fixed = -1);  // fixed: -1 = by v_mode
 // vgram.cu
 kldi_status vsched_upload(kldi_plan* P, const std::vector<int32_t>& h_kp, const std::vector<int32_t>& h_sh_ao0);
 }  // namespace kldi

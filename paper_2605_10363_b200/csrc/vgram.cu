@@ -378,7 +378,7 @@ static kldi_status launch_fx_bound(kldi_plan* P, bool gga) {
 }
 
 template <bool GGA, int EPI>
-static kldi_status launch_vgram(kldi_plan* P) {
+static kldi_status launch_vgram(kldi_plan* P, const double* phi_v = nullptr) {
   static bool attr_done = false;
   if (!attr_done) {
     KLDI_CUDA(cudaFuncSetAttribute(k_vgram<GGA, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, vg::SMEM_BYTES));
@@ -387,7 +387,8 @@ static kldi_status launch_vgram(kldi_plan* P) {
   const int m = GGA ? 1 : 0;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   k_vgram<GGA, EPI><<<grid, 32 * (V_WARPS + 1), vg::SMEM_BYTES, P->stream>>>(
-      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi_v, P->d_z, P->d_wv_s,
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, phi_v ? phi_v : P->d_phi_v, P->d_z,
+      P->d_wv_s,
       P->d_vsched_ptr[m], static_cast<const VPass*>(P->d_vpasses[m]), static_cast<const VItem*>(P->d_vitems[m]),
       P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram, P->d_fx);
   KLDI_CUDA(cudaGetLastError());
@@ -521,6 +522,34 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
   kldi_status rc = gga ? launch_vgram<true, 1>(P) : launch_vgram<false, 1>(P);
   if (rc != KLDI_OK) return rc;
   return gga ? launch_vreduce<true>(P) : launch_vreduce<false>(P);
+}
+
+// rho layout ([column][128 rows]) -> V layout (vlayout_off) of one store; HBM-bound.
+__global__ void __launch_bounds__(128) k_relayout_v(const int64_t* __restrict__ panel_off,
+                                                    const double* __restrict__ src, double* __restrict__ dst) {
+  const int p = blockIdx.x, t = threadIdx.x;
+  const int64_t base = panel_off[p];
+  const int K8 = (int)(panel_off[p + 1] - base);
+  for (int k = 0; k < K8; ++k) dst[vlayout_off(base, K8, k, t)] = src[(base + k) * GB + t];
+}
+
+// V^tau = 1/2 sum_c (d_c Phi)^T diag(wv) (d_c Phi): three LDA-form Gram builds that accumulate
+// into the same plan-order V; wv_s already carries the 1/2.  Each gradient store is first copied into the V layout
+// (the Z buffer serves as the scratch store).  Mode 1 (workspace + reduce) does not accumulate across launches, so it
+// runs as mode 2 here, which is reproducible and free of FP64 atomics as well.
+kldi_status launch_vtau(kldi_plan* P) {
+  KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  kldi_status rc;
+  if (P->v_mode != 0 && (rc = launch_fx_bound(P, false)) != KLDI_OK) return rc;
+  for (int c = 0; c < 3; ++c) {
+    k_relayout_v<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_panel_off, P->d_dphi[c], P->d_z);
+    KLDI_CUDA(cudaGetLastError());
+    KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+    rc = P->v_mode != 0 ? launch_vgram<false, 2>(P, P->d_z) : launch_vgram<false, 0>(P, P->d_z);
+    if (rc != KLDI_OK) return rc;
+  }
+  return KLDI_OK;
 }
 
 }  // namespace kldi

@@ -457,3 +457,47 @@ def test_exc_host_equals_device_path_and_reads_lower_triangle_only(K, n):
     E2, V2 = plan.exc(Dn)
     assert E2 == E0 and torch.equal(V2, V0)
     plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 2])
+@pytest.mark.parametrize("name,n", [("cfg0", None), ("cfg1", 8), ("cfg4", 6)])
+def test_tau_and_vtau_parity(K, name, n, mode):
+    """kldi_eval_tau / kldi_build_vtau (the rho and V contractions on the stored AO gradients)
+    against the oracle's plain definitions, element by element, same bar as rho and V; V^tau exactly symmetric, and
+    bitwise reproducible in the fixed-point mode."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional="lda")
+    plan = K.Plan.from_workload(wl, want_gradients=True)
+    plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, mode)
+    D = torch.as_tensor(wl.D, device="cuda")
+    tau = plan.eval_tau(D).cpu().numpy()
+    rng = np.random.default_rng(3)
+    wv = wl.grid_w * rng.uniform(-1.0, 1.0, size=wl.n_pts)          # w * v_tau with an arbitrary v_tau of both signs
+    Vt = plan.build_vtau(torch.as_tensor(wv, device="cuda"))
+    tau_ref = np.empty(wl.n_pts)
+    V_ref = np.zeros((wl.n_ao, wl.n_ao))
+    for c0 in range(0, wl.n_pts, 8192):
+        _, dphi = O.ao_values(*basis_of(wl), wl.grid_xyz[c0:c0 + 8192], deriv=True)
+        tau_ref[c0:c0 + 8192] = O.kinetic_energy_density(dphi, wl.D)
+        V_ref += O.vtau_from_wv(dphi, wv[c0:c0 + 8192])
+    assert np.max(np.abs(tau_ref)) > 1e-2
+    assert np.max(np.abs(tau - tau_ref)) <= TOL_RHO, np.max(np.abs(tau - tau_ref))
+    Vn = Vt.cpu().numpy()
+    assert np.max(np.abs(Vn - V_ref)) <= TOL_V, np.max(np.abs(Vn - V_ref))
+    assert np.array_equal(Vn, Vn.T)
+    if mode == 2:
+        V2 = plan.build_vtau(torch.as_tensor(wv, device="cuda"))
+        assert torch.equal(V2, Vt)
+    # the energy / potential path of the same plan is untouched by the scratch use of the Z store
+    E, V = plan.exc(D, K.KLDI_GGA_PBEX)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "gga")
+    assert abs(E - ref["E"]) <= TOL_E and np.max(np.abs(V.cpu().numpy() - ref["V"])) <= TOL_V
+    plan.close()
+    if name == "cfg0" and mode == 0:
+        plan0 = K.Plan.from_workload(wl, want_gradients=False)
+        with pytest.raises(K.KldiError):
+            plan0.eval_tau(D)
+        with pytest.raises(K.KldiError):
+            plan0.build_vtau(torch.as_tensor(wv, device="cuda"))
+        plan0.close()
