@@ -299,6 +299,21 @@ def main():
                     "grad_contraction_gbs": col_bytes / (tg["vxc"] * 1e-3) / 1e9,
                     "grad_contraction_frac_of_hbm": col_bytes / (tg["vxc"] * 1e-3) / 1e9 / peaks().get("hbm_gbs", 6650.0),
                     "sum_k": sg["sum_k"], "plan_create_s": sg["plan_seconds"]}
+        # the meta-GGA contractions on the same plan (three LDA-form builds each)
+        wv_t = torch.as_tensor(wl.grid_w, device="cuda").clone()
+        Vt = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")
+        t_tau, t_vtau = [], []
+        for i in range(3 + min(args.steps, 10)):
+            plan_g.eval_tau(D)
+            a = plan_g.last_timings()["rho"]
+            plan_g.build_vtau(wv_t, out=Vt)
+            b = plan_g.last_timings()["vxc"]
+            if i >= 3:
+                t_tau.append(a)
+                t_vtau.append(b)
+        grad_leg["meta_gga"] = {"eval_tau_ms": float(np.median(t_tau)), "build_vtau_ms": float(np.median(t_vtau)),
+                                "tau_tflops_useful": 3 * sg["flops_rho_useful_sym"] / (np.median(t_tau) * 1e-3) / 1e12,
+                                "vtau_tflops_useful": 3 * sg["flops_rho_useful_sym"] / (np.median(t_vtau) * 1e-3) / 1e12}
         plan_g.close()
 
     if rank != 0:
