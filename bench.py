@@ -273,6 +273,37 @@ def main():
                   "bitwise_equal_between_calls": bool(torch.equal(Va, V))}
         plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 0)
 
+    # ---- BASELINE.json configs[3]: how the retained fraction, the throughput and the result move with eps.  The
+    # differences are taken against this run's eps (GPU vs GPU: the screening increment; oracle parity is in tests/).
+    eps_leg = None
+    if world == 1 and args.config == "cfg3" and abs(args.eps - 1e-12) < 1e-20:
+        rho_a = plan.eval_rho(D).clone()
+        Ea, _ = plan.exc(D, func, out=V)
+        Va = V.clone()
+        eps_leg = []
+        for eps2 in (1e-10, 1e-8):
+            p2 = K.Plan.from_workload(wl, eps=eps2)
+            V2 = torch.empty_like(V)
+            for _ in range(3):
+                E2, _ = p2.exc(D, func, out=V2)
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            q0.record()
+            for _ in range(5):
+                p2.exc(D, func, out=V2)
+            q1.record()
+            torch.cuda.synchronize()
+            s2 = p2.stats.as_dict()
+            eps_leg.append({"eps": eps2, "evals_per_s": 5e3 / q0.elapsed_time(q1),
+                            "retained_blocks_over_candidates": s2["retained_blocks"] / s2["candidate_blocks"],
+                            "sum_k": s2["sum_k"], "phi_bytes": s2["phi_bytes"],
+                            "retained_over_dense_flops": (s2["flops_rho_useful_sym"] + s2["flops_v_useful"]) / (2 * s2["flops_dense"]),
+                            "max_abs_d_rho_vs_eps1e-12": float((p2.eval_rho(D) - rho_a).abs().max()),
+                            "max_abs_d_V_vs_eps1e-12": float((V2 - Va).abs().max()),
+                            "abs_d_E_vs_eps1e-12": abs(E2 - Ea)})
+            p2.close()
+        del rho_a, Va
+
     # ---- the LDA nuclear-gradient contraction on the same molecule (its own plan: Phi + grad Phi)
     grad_leg = None
     if args.grad and world == 1:
@@ -383,7 +414,7 @@ def main():
         "pair_test": {"enabled": bool(args.pair_test), "stages_total": plan.refresh_stats().pair_stages_total,
                       "stages_executed": plan.stats.pair_stages_executed},
         "gpu_launches": 6 + (1 if gga else 0) + {0: 0, 1: 1, 2: 2}[args.deterministic_v] + 2 * args.pair_test, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
-        "nuclear_gradient": grad_leg, "reproducible_v": fx_leg,
+        "nuclear_gradient": grad_leg, "reproducible_v": fx_leg, "eps_scaling": eps_leg,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)
