@@ -24,8 +24,8 @@ int rho = Tr(D S); closed-form Slater energy of one s-Gaussian; V symmetric; cen
 differences dE/dD = V (LDA and PBE-x); brute-force loops on single water; PBE-x limits; central finite
 differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda; kinetic-energy density: closed
 form int tau = 3 alpha n / 2 of one s-Gaussian, AO gradients from finite differences, Tr(D V^tau) = sum wv tau.
-Absolute PBE-x energies have no printed reference value: beyond the limits and the FD
-identity they are "parity unpinned".
+Absolute PBE-x (and Slater) energies: the four decimals the PBE paper prints for the exchange energy of
+the hydrogen atom (tests/golden/pbe_x_hydrogen.txt), by a 1-D radial integral of slater() / pbe_x().
 """
 from __future__ import annotations
 

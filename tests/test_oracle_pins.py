@@ -193,6 +193,33 @@ def test_kinetic_energy_density_and_vtau(water):
     assert abs(loop - Vt[m, k]) < 1e-13 * np.max(np.abs(Vt))
 
 
+def test_exchange_energy_of_the_hydrogen_atom_matches_the_literature():
+    """Absolute pin of the functionals: the oracle's slater() and pbe_x() integrated over the exact hydrogen 1s density
+    (a 1-D radial integral by scipy's quad — none of the AO / grid machinery) reproduce the four decimals printed in
+    the PBE paper's Table I (tests/golden/pbe_x_hydrogen.txt).  A wrong C_x, mu, kappa, a factor in the reduced
+    gradient s^2 = sigma / (4 (3 pi^2)^{2/3} rho^{8/3}) or in sigma moves the PBE value in the third decimal."""
+    from scipy import integrate
+
+    gold = np.loadtxt(os.path.join(HERE, "golden", "pbe_x_hydrogen.txt"))
+
+    def e_x(kind):
+        def integrand(r):
+            rho = 2.0 * np.exp(-2.0 * r) / np.pi            # 2 rho_up (spin scaling)
+            grad = 2.0 * rho                                # |d rho / d r| of exp(-2r)
+            if kind == 0:
+                e = O.slater(np.array([rho]))[0]
+            else:
+                e = O.pbe_x(np.array([rho]), np.array([grad * grad]))[0]
+            return 4.0 * np.pi * r * r * float(e[0])
+        return 0.5 * integrate.quad(integrand, 0.0, 40.0, epsabs=1e-12, epsrel=1e-12, limit=400)[0]
+
+    for kind, ref in gold:
+        assert abs(e_x(int(kind)) - ref) < 5e-5, (kind, e_x(int(kind)), ref)
+    # closed form of the LSD value: -C_x 2^{1/3} int rho_up^{4/3} d^3r, int (e^{-2r}/pi)^{4/3} 4 pi r^2 dr = 4 pi^{-1/3} 2/(8/3)^3
+    closed = -0.75 * (3.0 / np.pi) ** (1.0 / 3.0) * 2.0 ** (1.0 / 3.0) * 4.0 * np.pi * np.pi ** (-4.0 / 3.0) * 2.0 / (8.0 / 3.0) ** 3
+    assert abs(e_x(0) - closed) < 1e-10
+
+
 def test_pbe_enhancement_limits():
     rho = np.geomspace(1e-12, 50.0, 200)
     e_s, v_s = O.slater(rho)
