@@ -92,7 +92,7 @@ typedef struct {
   double flops_rho_useful;  /* sum_p 2*128*K_p^2: retained-block FLOPs of one rho build without symmetry (GGA form) */
   double flops_rho_exec;    /* FLOPs the GGA-form rho kernel issues (K_p padded to 8) */
   double flops_v_useful;    /* LDA: sum_p 128*K_p*(K_p+1) (q<=r only); GGA: sum_p 2*128*K_p^2 */
-  double flops_v_exec;      /* FLOPs the V kernel issues (16 x 8 MMA units of the schedule, padded) */
+  double flops_v_exec;      /* FLOPs the V kernel issues (the 8 x 8 blocks of its schedule, K_p padded to 8) */
   double flops_dense;       /* 2*n_pts*n_ao^2 : one dense product */
   double plan_seconds;      /* wall time of kldi_plan_create */
   double eps;

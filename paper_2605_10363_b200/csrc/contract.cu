@@ -2,12 +2,14 @@
 //   H1 k_permute_D   — D in plan AO order
 //   H2 k_rho         — X_p = Phi_p D[L(p),L(p)], rho_p = rowsum(Phi_p o X_p) (Eq. 4/18)
 //   H3 k_xc          — Slater / PBE-x per point, wv = w v, deterministic energy reduction (Eq. 1/3)
-//   H4 k_vxc         — G_p = Phi_p^T diag(wv_p) Phi_p scattered into V (Eq. 5/16)
+//   H4 k_vgram       — G_p = Phi_p^T diag(wv_p) Phi_p scattered into V (Eq. 5/16): vgram.cu
 //   H5 k_finalise_V  — mirror / symmetrise, back to caller AO order
-// H2 and H4 are persistent, warp-specialised kernels: one producer warp pulls grid-block tasks
-// from an atomic ticket (the paper's pull-based pool, on-device) and streams
-// operand tiles through an mbarrier ring with bulk-async copies (TMA engine) and 8-byte cp.async;
-// eight consumer warps issue FP64 tensor-core MMAs (DMMA.8x8x4) on register accumulators.
+//   F2 k_grad_cols   — LDA nuclear-gradient contraction from the X store k_rho writes
+//   F4 k_tau_combine — kinetic-energy density from three LDA-form k_rho builds on the gradient stores (§8(f4))
+// H2 and H4 are persistent, warp-specialised kernels: producer warps pull grid-block tasks from an atomic
+// ticket (the paper's pull-based pool, on-device) and stream operand tiles through an mbarrier
+// ring with bulk-async copies (TMA engine) and 8-byte cp.async; 16 (k_rho) / 15 (k_vgram) consumer warps issue
+// FP64 tensor-core MMAs (DMMA.8x8x4) on register accumulators.
 #include <cstdio>
 
 #include "kldi_internal.h"
