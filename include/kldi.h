@@ -215,6 +215,12 @@ kldi_status kldi_fp64_peak(int kind, int iters, double* tflops);
  * to [0, 2^20-1].  xyz, origin: HOST [3]. */
 uint64_t kldi_morton_key(const double* xyz, const double* origin);
 
+/* The key the plan sorts the grid points (and the atoms) by, on the host, no GPU needed: the Hilbert-curve index of the
+ * same three 20-bit lattice coordinates as Eq. 20 (Skilling's transform, then Eq. 20's bit interleave) — SURVEY.md
+ * §8(f1): no jumps along the curve, so blocks of 128 consecutive points are more compact than with the Z-order and
+ * retain fewer AO shells.  The order is internal; results do not depend on it.  xyz, origin: HOST [3]. */
+uint64_t kldi_grid_key(const double* xyz, const double* origin);
+
 /* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
  * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32
  * {c1_lo, c1_n, c2_lo, c2_n, max_load (of a warp), units, smsp_load (max over the 4 scheduler partitions w % 4), n_warps | n_slots << 8}; items: [cap][32][2] int32 (item

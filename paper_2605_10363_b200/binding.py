@@ -21,7 +21,7 @@ KLDI_GGA_PBEX = 1
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_exc_grad", "kldi_eval_tau", "kldi_build_vtau", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
-    "kldi_morton_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
+    "kldi_morton_key", "kldi_grid_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
     "kldi_vlayout_offset",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
@@ -91,12 +91,14 @@ def lib():
         L.kldi_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.kldi_morton_key.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.kldi_morton_key.restype = C.c_uint64
+        L.kldi_grid_key.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.kldi_grid_key.restype = C.c_uint64
         L.kldi_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.kldi_vsched_export.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_vlayout_offset.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         L.kldi_vlayout_offset.restype = C.c_int64
         for name in EXPORTED:
-            if name not in ("kldi_last_error", "kldi_morton_key", "kldi_vlayout_offset"):
+            if name not in ("kldi_last_error", "kldi_morton_key", "kldi_grid_key", "kldi_vlayout_offset"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -286,6 +288,13 @@ def morton_key(xyz, origin) -> int:
     a = (C.c_double * 3)(*[float(v) for v in xyz])
     o = (C.c_double * 3)(*[float(v) for v in origin])
     return int(lib().kldi_morton_key(a, o))
+
+
+def grid_key(xyz, origin) -> int:
+    """Host evaluation of the key the plan sorts by (Hilbert index of Eq. 20's lattice coordinates)."""
+    a = (C.c_double * 3)(*[float(v) for v in xyz])
+    o = (C.c_double * 3)(*[float(v) for v in origin])
+    return int(lib().kldi_grid_key(a, o))
 
 
 def vsched(nb: int, square: bool = False):

@@ -78,6 +78,11 @@ uint64_t kldi_morton_key(const double* xyz, const double* origin) {
   return morton_key_host(xyz[0], xyz[1], xyz[2], origin[0], origin[1], origin[2]);
 }
 
+uint64_t kldi_grid_key(const double* xyz, const double* origin) {
+  if (!xyz || !origin) return ~0ull;
+  return grid_key_host(xyz[0], xyz[1], xyz[2], origin[0], origin[1], origin[2]);
+}
+
 kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid, double eps,
                              int want_gradients, void* cuda_stream, kldi_plan** out) {
   if (out) *out = nullptr;

@@ -129,6 +129,7 @@ struct kldi_plan {
 namespace kldi {
 // plan.cu
 uint64_t morton_key_host(double x, double y, double z, double x0, double y0, double z0);
+uint64_t grid_key_host(double x, double y, double z, double x0, double y0, double z0);
 kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid);
 void plan_free(kldi_plan* P);
 // contract.cu

@@ -107,6 +107,39 @@ def test_morton_key_is_eq20(lib):
     assert binding.morton_key([0.5001, 0.2501, 0.1251], [0, 0, 0]) == binding.morton_key([0.5003, 0.2503, 0.1253], [0, 0, 0])
 
 
+def test_grid_key_is_a_hilbert_curve(lib):
+    """kldi_grid_key (the key the plan sorts by): a bijection of the 2^20-per-axis lattice onto
+    60-bit indices whose successive cells are face neighbours (no jumps: what makes blocks of consecutive points
+    compact), nested (the first 3 L index bits fix the cell at level L), clamped like Eq. 20."""
+    from paper_2605_10363_b200 import binding
+
+    for level in (1, 2, 3, 4):                     # the 2^level cube of cells, each 2^(20-level) lattice units wide
+        n, side = 2 ** level, 2 ** (20 - level)
+        cells = [(i, j, k) for i in range(n) for j in range(n) for k in range(n)]
+        keys = {}
+        for c in cells:
+            lo = binding.grid_key([v * side / 128.0 for v in c], [0, 0, 0]) >> (60 - 3 * level)
+            hi = binding.grid_key([((v + 1) * side - 1) / 128.0 + 1e-9 for v in c], [0, 0, 0]) >> (60 - 3 * level)
+            assert lo == hi                        # nested: every lattice point of the cell shares the index prefix
+            keys[lo] = c
+        assert sorted(keys) == list(range(n ** 3))  # bijection at this level
+        path = [keys[i] for i in range(n ** 3)]
+        assert all(sum(abs(a - b) for a, b in zip(p, q)) == 1 for p, q in zip(path, path[1:]))
+    # full-resolution neighbours along the curve, around an arbitrary point
+    rng = np.random.default_rng(7)
+    seen = set()
+    for _ in range(200):
+        q = rng.integers(0, 2 ** 20, 3)
+        k = binding.grid_key([(v + 0.5) / 128.0 for v in q], [0, 0, 0])
+        assert 0 <= k < 2 ** 60 and k not in seen
+        seen.add(k)
+        nb = [binding.grid_key([(v + 0.5 + d * (a == ax)) / 128.0 for a, v in enumerate(q)], [0, 0, 0])
+              for ax in range(3) for d in (-1, 1) if 0 <= q[ax] + d < 2 ** 20]
+        assert sum(abs(m - k) == 1 for m in nb) >= 1 or k in (0, 2 ** 60 - 1)   # predecessor or successor is a face neighbour
+    assert binding.grid_key([-5.0, -5.0, -5.0], [0, 0, 0]) == binding.grid_key([0, 0, 0], [0, 0, 0]) == 0
+    assert binding.grid_key([1e9, 1e9, 1e9], [0, 0, 0]) == binding.grid_key([8192.0, 8192.0, 8192.0], [0, 0, 0])
+
+
 @pytest.mark.parametrize("square", [False, True])
 def test_v_schedule_covers_every_unit_once(square):
     """Host logic of the V contraction (csrc/vsched.h): for every panel size the passes tile the (16-row strip,

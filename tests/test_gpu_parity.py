@@ -136,7 +136,8 @@ def test_eval_rho_and_build_vxc_separately(K):
 
 
 def test_plan_structure_invariants(K):
-    """Eq. 20 ordering and the lossless BCS(R)/BCS(C) re-layout."""
+    """Spatial ordering (Hilbert index of Eq. 20's lattice coordinates, stable sort) and the lossless BCS(R)/BCS(C)
+    re-layout (PAPER.md:438-442, 459-471)."""
     wl = W.named_config("cfg1", n_override=5)
     plan = K.Plan.from_workload(wl)
     perm = plan.export("perm_g")
@@ -148,8 +149,8 @@ def test_plan_structure_invariants(K):
     assert np.all(perm[wl.n_pts:] == -1)                               # padding last
     assert np.all(np.diff(keys.astype(np.float64)) >= 0) and np.all(keys[:wl.n_pts][1:] >= keys[:wl.n_pts][:-1])
     origin = wl.grid_xyz.min(axis=0)
-    for i in np.random.default_rng(0).integers(0, wl.n_pts, 200):       # keys are Eq. 20 of the sorted points
-        assert int(keys[i]) == K.morton_key(wl.grid_xyz[perm[i]], origin)
+    for i in np.random.default_rng(0).integers(0, wl.n_pts, 200):       # keys are kldi_grid_key of the sorted points
+        assert int(keys[i]) == K.grid_key(wl.grid_xyz[perm[i]], origin)
     same = keys[:wl.n_pts][1:] == keys[:wl.n_pts][:-1]                   # stable sort: ties keep caller order
     assert np.all(perm[:wl.n_pts][1:][same] > perm[:wl.n_pts][:-1][same])
     row_ptr, col_idx = plan.export("row_ptr"), plan.export("col_idx")
