@@ -157,6 +157,8 @@ def main():
                     help="1: executable-pair selection a_pq*b_qr >= eps per call (Eq. 17-19)")
     ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1, 2],
                     help="V without FP64 atomics: 1 = workspace partials + fixed-order reduce, 2 = fixed-point integer atomics")
+    ap.add_argument("--rho-dfma", type=int, default=0, choices=[0, 1],
+                    help="1: LDA rho contraction on the vector FP64 pipe (register tiles) instead of DMMA tiles")
     ap.add_argument("--grad", action="store_true",
                     help="also time kldi_exc_grad (LDA nuclear-gradient contraction) on a plan with gradient stores")
     args = ap.parse_args()
@@ -198,6 +200,7 @@ def main():
     plan = K.Plan.from_workload(wl)
     plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
     plan.set_option(K.KLDI_OPT_PAIR_TEST, args.pair_test)
+    plan.set_option(K.KLDI_OPT_RHO_DFMA, args.rho_dfma)
     st = plan.stats.as_dict()
     D = torch.as_tensor(wl.D, device="cuda")
     V = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")

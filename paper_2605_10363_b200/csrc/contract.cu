@@ -144,8 +144,145 @@ __device__ __forceinline__ void rho_stage(double (&acc)[16][2], const double* __
   }
 }
 
-template <bool GGA, bool TRI>
-__global__ void __launch_bounds__(rho::NTHREADS, 1)
+// ------------------------------------------------------------------------------------ DFMA consumer (IMPL = 1)
+// DMMA.8x8x4 tops out at 80 % of the FP64 unit rate on this part (profiles/r1f_summary.md); plain DFMA does not.  This
+// consumer runs the LDA (triangular D') rho build on the vector pipe with register tiles: 8 consumer warps, lane l owns
+// grid rows 2l, 2l+1, 64+2l, 64+2l+1 (two conflict-free 16-byte loads per Phi column), warp w owns the column PAIRS q = w, w+8, w+16, ... of the N-tile (columns 16t + 2w + {0,1}: cyclic,
+// so that the triangular shape of D' loads every warp alike), tile width <= 96 -> 4 x 12 accumulators per lane.  Per k:
+// two 16-byte loads of Phi (the lane's rows of column k), one 16-byte broadcast load of D'[k][pair] per pair, 8 DFMA per
+// pair.  The producer side, the ring and the stage headers are those of the DMMA kernel.
+namespace rho {
+constexpr int NCW_F = 8, TW_F = 96, NTP_F = TW_F / 16;   // consumer warps, tile width, pair slots per warp
+constexpr int RED_OFF = (SMEM_BYTES + 15) & ~15;         // [8 warps][128 rows] partial row sums of a panel
+constexpr int SMEM_BYTES_F = RED_OFF + NCW_F * GB * 8;
+}  // namespace rho
+
+template <int NTS>  // pair slots 0..NTS-1 of this warp are inside the rectangle
+__device__ __forceinline__ void rho_f_rect(double (&acc)[4][2 * rho::NTP_F], const double* __restrict__ pa,
+                                           const double* __restrict__ db, int kc) {
+#pragma unroll 2
+  for (int k = 0; k < kc; ++k) {
+    const double2 a01 = *reinterpret_cast<const double2*>(pa + k * LD);
+    const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 64);
+#pragma unroll
+    for (int t = 0; t < NTS; ++t) {
+      const double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * t);
+      acc[0][2 * t] = fma(a01.x, b.x, acc[0][2 * t]);
+      acc[0][2 * t + 1] = fma(a01.x, b.y, acc[0][2 * t + 1]);
+      acc[1][2 * t] = fma(a01.y, b.x, acc[1][2 * t]);
+      acc[1][2 * t + 1] = fma(a01.y, b.y, acc[1][2 * t + 1]);
+      acc[2][2 * t] = fma(a23.x, b.x, acc[2][2 * t]);
+      acc[2][2 * t + 1] = fma(a23.x, b.y, acc[2][2 * t + 1]);
+      acc[3][2 * t] = fma(a23.y, b.x, acc[3][2 * t]);
+      acc[3][2 * t + 1] = fma(a23.y, b.y, acc[3][2 * t + 1]);
+    }
+  }
+}
+
+// The chunk's own columns [o0, o0 + kc) of the tile (o0 = 16 T0): this warp's pairs there are slots T0 and T0 + 1,
+// columns c = 16 t + 2 w; D'[k][c] = 0 for chunk rows k < c - o0, so the pair starts at k = c - o0.  After the chunk
+// these columns of X' are final and their Phi columns are the chunk's own columns c - o0 of the stage: epilogue.
+template <int T0>
+__device__ __forceinline__ void rho_f_diag(double (&acc)[4][2 * rho::NTP_F], double (&rs)[4],
+                                           const double* __restrict__ pa, const double* __restrict__ db, int kc, int w) {
+#pragma unroll
+  for (int tt = 0; tt < 2; ++tt) {
+    constexpr int dummy = 0;
+    (void)dummy;
+    const int t = T0 + tt;
+    if (T0 + tt < rho::NTP_F) {
+      const int ks = 16 * tt + 2 * w;  // first chunk row that reaches this pair
+      if (ks < kc) {
+        for (int k = ks; k < kc; ++k) {
+          const double2 a01 = *reinterpret_cast<const double2*>(pa + k * LD);
+          const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 64);
+          const double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * t);
+          acc[0][2 * (T0 + tt)] = fma(a01.x, b.x, acc[0][2 * (T0 + tt)]);
+          acc[0][2 * (T0 + tt) + 1] = fma(a01.x, b.y, acc[0][2 * (T0 + tt) + 1]);
+          acc[1][2 * (T0 + tt)] = fma(a01.y, b.x, acc[1][2 * (T0 + tt)]);
+          acc[1][2 * (T0 + tt) + 1] = fma(a01.y, b.y, acc[1][2 * (T0 + tt) + 1]);
+          acc[2][2 * (T0 + tt)] = fma(a23.x, b.x, acc[2][2 * (T0 + tt)]);
+          acc[2][2 * (T0 + tt) + 1] = fma(a23.x, b.y, acc[2][2 * (T0 + tt) + 1]);
+          acc[3][2 * (T0 + tt)] = fma(a23.y, b.x, acc[3][2 * (T0 + tt)]);
+          acc[3][2 * (T0 + tt) + 1] = fma(a23.y, b.y, acc[3][2 * (T0 + tt) + 1]);
+        }
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {  // epilogue: X'[rows][c + e] . Phi[rows][c + e], Phi column = chunk column ks + e
+          const double2 p01 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD);
+          const double2 p23 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD + 64);
+          rs[0] = fma(acc[0][2 * (T0 + tt) + e], p01.x, rs[0]);
+          rs[1] = fma(acc[1][2 * (T0 + tt) + e], p01.y, rs[1]);
+          rs[2] = fma(acc[2][2 * (T0 + tt) + e], p23.x, rs[2]);
+          rs[3] = fma(acc[3][2 * (T0 + tt) + e], p23.y, rs[3]);
+        }
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void rho_consumer_dfma(unsigned char* smem, const int* hdr, uint32_t bar0,
+                                                  double* __restrict__ rho_s, int warp, int lane) {
+  using namespace rho;
+  double acc[4][2 * NTP_F];
+  double rs[4] = {0.0, 0.0, 0.0, 0.0};
+  double* red = reinterpret_cast<double*>(smem + RED_OFF);
+  int s = 0;
+  uint32_t ph = 0;
+  for (;;) {
+    mbar_wait(bar0 + 8 * s, ph);
+    const int p = hdr[4 * s + 0], h2 = hdr[4 * s + 2], h3 = hdr[4 * s + 3];
+    const int fl = h2 >> 16;
+    if (fl & F_DONE) break;
+    const int kc = (h2 & 0xff) * 4, wact = ((h2 >> 8) & 0xff) * 8, ecnt = h3 >> 16, o0 = ((h3 >> 8) & 0xff) * 8;
+    if (fl & F_FIRST) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 2 * NTP_F; ++j) acc[i][j] = 0.0;
+    }
+    const double* pa = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * lane;            // rows of column k
+    const double* db = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + 2 * warp;  // pair slot 0
+    const int cw = ecnt ? o0 : wact;                                  // width of the rectangle before the own columns
+    const int nts = cw > 2 * warp ? (cw - 2 * warp + 15) >> 4 : 0;    // this warp's pair slots inside it
+    switch (nts) {
+      case 1: rho_f_rect<1>(acc, pa, db, kc); break;
+      case 2: rho_f_rect<2>(acc, pa, db, kc); break;
+      case 3: rho_f_rect<3>(acc, pa, db, kc); break;
+      case 4: rho_f_rect<4>(acc, pa, db, kc); break;
+      case 5: rho_f_rect<5>(acc, pa, db, kc); break;
+      case 6: rho_f_rect<6>(acc, pa, db, kc); break;
+      default: break;
+    }
+    if (ecnt) {
+      switch (o0 >> 5) {
+        case 0: rho_f_diag<0>(acc, rs, pa, db, kc, warp); break;
+        case 1: rho_f_diag<2>(acc, rs, pa, db, kc, warp); break;
+        default: rho_f_diag<4>(acc, rs, pa, db, kc, warp); break;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+    if (++s == NST) { s = 0; ph ^= 1; }
+
+    if (fl & F_LAST_PANEL) {  // rho_p: fixed-order sum of the 8 warps' partial row sums
+      *reinterpret_cast<double2*>(red + warp * GB + 2 * lane) = make_double2(rs[0], rs[1]);
+      *reinterpret_cast<double2*>(red + warp * GB + 64 + 2 * lane) = make_double2(rs[2], rs[3]);
+      rs[0] = rs[1] = rs[2] = rs[3] = 0.0;
+      asm volatile("bar.sync 2, %0;" ::"n"(32 * NCW_F) : "memory");
+      const int r = warp * 32 + lane;
+      if (r < GB) {
+        double v = 0.0;
+#pragma unroll
+        for (int w2 = 0; w2 < NCW_F; ++w2) v += red[w2 * GB + r];
+        rho_s[(int64_t)p * GB + r] = 2.0 * v;
+      }
+      asm volatile("bar.sync 2, %0;" ::"n"(32 * NCW_F) : "memory");
+    }
+  }
+}
+
+template <bool GGA, bool TRI, int IMPL = 0>
+__global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTHREADS, 1)
     k_rho(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
           const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
@@ -153,6 +290,9 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
           double* __restrict__ drho_s, int64_t n_pad, const unsigned long long* __restrict__ pmask,
           double* __restrict__ x_store) {
   using namespace rho;
+  static_assert(IMPL == 0 || (TRI && !GGA), "the DFMA consumer implements the LDA (triangular) form");
+  constexpr int NCWI = IMPL ? NCW_F : NCW;  // consumer warps
+  constexpr int TW = IMPL ? TW_F : NT;      // N-tile width
   extern __shared__ __align__(128) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
   const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);  // full[s] at +8s, empty[s] at +8(NST+s)
@@ -160,15 +300,15 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) {
       mbar_init(bar0 + 8 * s, 1 + 32 * NPW);  // expect_tx arrive + one cp.async completion per producer lane
-      mbar_init(bar0 + 8 * (NST + s), NCW);  // one arrive per consumer warp
+      mbar_init(bar0 + 8 * (NST + s), NCWI);  // one arrive per consumer warp
     }
     fence_mbar_init();
   }
   __syncthreads();
 
-  if (warp >= NCW) {
+  if (warp >= NCWI) {
     // ------------------------------------------------------------------ producer warps (in lockstep per task)
-    const int pw = warp - NCW;
+    const int pw = warp - NCWI;
     volatile int* task_slot = reinterpret_cast<volatile int*>(smem + NST * STAGE_BYTES + NST * 16 + 2 * NST * 8);
     int s = 0;
     uint32_t ph = 0;
@@ -181,7 +321,7 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
       const int p = tasks[t];
       const int K8 = (kp[p] + 7) & ~7;
       const int64_t base = panel_off[p];
-      const int ntile = (K8 + NT - 1) / NT;
+      const int ntile = (K8 + TW - 1) / TW;
       // executable-pair mask of this grid block (pairsel.cu; Eq. 19): bit (k0/32)*4 + jt, all ones = no test
       const unsigned long long pm = pmask ? pmask[p] : ~0ull;
       // TRI: tiles start on 32-column (K-chunk) boundaries so that a chunk's own columns are whole j-groups
@@ -280,6 +420,10 @@ __global__ void __launch_bounds__(rho::NTHREADS, 1)
     return;
   }
 
+  if constexpr (IMPL == 1) {
+    rho_consumer_dfma(smem, hdr, bar0, rho_s, warp, lane);
+    return;
+  }
   // -------------------------------------------------------------------- consumer warps (8 rows each)
   double acc[16][2];
   double rs[GGA ? 4 : 1];
@@ -524,6 +668,7 @@ static kldi_status set_attrs() {
   if (g_attr_done) return KLDI_OK;
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES_F));
   g_attr_done = 1;
   return KLDI_OK;
 }
@@ -556,6 +701,10 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
                                                            P->n_pad, pm, x_store);
+  else if (P->rho_impl == 1 && !pm)
+    k_rho<false, true, 1><<<grid, 32 * (rho::NCW_F + rho::NPW), rho::SMEM_BYTES_F, P->stream>>>(
+        P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr, nullptr,
+        P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad, nullptr, nullptr);
   else
     k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp,
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,

@@ -97,6 +97,7 @@ struct kldi_plan {
   double* d_gram = nullptr;                       // lazily allocated workspace of G_p partials
   int64_t gram_cap = 0;
   int32_t* d_ao_shell = nullptr;                  // plan AO -> plan shell
+  int rho_impl = 0;                               // LDA rho build: 0 DMMA tiles, 1 DFMA register tiles (KLDI_OPT_RHO_DFMA)
   int v_mode = 0;                                 // 0: red.global.add.f64 epilogue, 1: workspace + fixed-order reduce,
                                                   // 2: 64-bit fixed-point integer atomics (reproducible)
   double* d_fx = nullptr;                         // [1 + n_blocks] fixed-point bound, then s_p = sum_g |wv_g| per block

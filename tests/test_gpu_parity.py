@@ -502,3 +502,27 @@ def test_tau_and_vtau_parity(K, name, n, mode):
         with pytest.raises(K.KldiError):
             plan0.build_vtau(torch.as_tensor(wv, device="cuda"))
         plan0.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg0", None), ("cfg1", 8), ("cfg2", 6), ("cfg3", 12)])
+def test_rho_dfma_option_parity(K, name, n):
+    """KLDI_OPT_RHO_DFMA: the LDA rho contraction on the vector FP64 pipe (register tiles, 96-column N-tiles, cyclic
+    column pairs) — same parity bar against the oracle, rho and E bitwise reproducible, and within rounding of the
+    DMMA path."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional="lda")
+    plan = K.Plan.from_workload(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    E0, V0 = plan.exc(D)
+    r0 = plan.eval_rho(D).clone()
+    plan.set_option(K.KLDI_OPT_RHO_DFMA, 1)
+    E1, V1 = plan.exc(D)
+    r1 = plan.eval_rho(D).clone()
+    E2, _ = plan.exc(D)
+    r2 = plan.eval_rho(D)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda")
+    check({"rho": r1.cpu().numpy(), "V": V1.cpu().numpy(), "E": E1, "drho": None}, ref)
+    assert E1 == E2 and torch.equal(r1, r2)
+    assert float((r1 - r0).abs().max()) <= 1e-12 * max(1.0, float(r0.abs().max()))
+    plan.close()
