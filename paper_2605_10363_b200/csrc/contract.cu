@@ -146,74 +146,87 @@ __device__ __forceinline__ void rho_stage(double (&acc)[16][2], const double* __
 
 // ------------------------------------------------------------------------------------ DFMA consumer (IMPL = 1)
 // DMMA.8x8x4 tops out at 80 % of the FP64 unit rate on this part (profiles/r1f_summary.md); plain DFMA does not.  This
-// consumer runs the LDA (triangular D') rho build on the vector pipe with register tiles: 8 consumer warps, lane l owns
-// grid rows 2l, 2l+1, 64+2l, 64+2l+1 (two conflict-free 16-byte loads per Phi column), warp w owns the column PAIRS q = w, w+8, w+16, ... of the N-tile (columns 16t + 2w + {0,1}: cyclic,
-// so that the triangular shape of D' loads every warp alike), tile width <= 96 -> 4 x 12 accumulators per lane.  Per k:
-// two 16-byte loads of Phi (the lane's rows of column k), one 16-byte broadcast load of D'[k][pair] per pair, 8 DFMA per
-// pair.  The producer side, the ring and the stage headers are those of the DMMA kernel.
+// consumer runs the LDA (triangular D') rho build on the vector pipe with register tiles.  8 consumer warps = 4 row
+// blocks (wr) x 2 column halves (wc); a lane is (g = lane / 4, h = lane % 4): rows 32 wr + {2g, 2g+1, 16+2g, 17+2g},
+// column owner o = 4 wc + h of the column PAIRS q = o, o+8, o+16, ... of the N-tile (columns 16 t + 2 o + {0,1}: cyclic,
+// so that the triangular shape of D' loads every owner alike); tile width <= 64 -> 4 x 8 accumulators per lane (96 spills
+// at the 170-register budget of 12 warps and ran slower).  Per k:
+// two 16-byte loads of Phi (8 row groups x 16 B: one wavefront, broadcast over h) and one 16-byte load of D'[k][pair]
+// per pair slot (4 owners x 16 B, broadcast over g), 8 DFMA per pair slot.  The producer side, the ring and the stage
+// headers are those of the DMMA kernel.
 namespace rho {
-constexpr int NCW_F = 8, TW_F = 96, NTP_F = TW_F / 16;   // consumer warps, tile width, pair slots per warp
-constexpr int RED_OFF = (SMEM_BYTES + 15) & ~15;         // [8 warps][128 rows] partial row sums of a panel
-constexpr int SMEM_BYTES_F = RED_OFF + NCW_F * GB * 8;
+#ifndef KLDI_TW_F
+#define KLDI_TW_F 64
+#endif
+constexpr int NCW_F = 8, TW_F = KLDI_TW_F, NTP_F = TW_F / 16;   // consumer warps, tile width, pair slots per owner
+constexpr int RED_OFF = (SMEM_BYTES + 15) & ~15;         // [2 column halves][128 rows] partial row sums of a panel
+constexpr int SMEM_BYTES_F = RED_OFF + 2 * GB * 8;
 }  // namespace rho
 
-template <int NTS>  // pair slots 0..NTS-1 of this warp are inside the rectangle
+__device__ __forceinline__ void rho_f_fma8(double (&acc)[4][2 * rho::NTP_F], int t, const double2& a01,
+                                           const double2& a23, const double2& b) {
+  acc[0][2 * t] = fma(a01.x, b.x, acc[0][2 * t]);
+  acc[0][2 * t + 1] = fma(a01.x, b.y, acc[0][2 * t + 1]);
+  acc[1][2 * t] = fma(a01.y, b.x, acc[1][2 * t]);
+  acc[1][2 * t + 1] = fma(a01.y, b.y, acc[1][2 * t + 1]);
+  acc[2][2 * t] = fma(a23.x, b.x, acc[2][2 * t]);
+  acc[2][2 * t + 1] = fma(a23.x, b.y, acc[2][2 * t + 1]);
+  acc[3][2 * t] = fma(a23.y, b.x, acc[3][2 * t]);
+  acc[3][2 * t + 1] = fma(a23.y, b.y, acc[3][2 * t + 1]);
+}
+
+// Rectangle [0, cw) of the stage's columns: NTS pair slots of the warp's first owner; an owner whose last slot lies
+// beyond cw multiplies zeros there (last_ok = 0).
+template <int NTS>
 __device__ __forceinline__ void rho_f_rect(double (&acc)[4][2 * rho::NTP_F], const double* __restrict__ pa,
-                                           const double* __restrict__ db, int kc) {
-#pragma unroll 2
+                                           const double* __restrict__ db, int kc, bool last_ok) {
+#pragma unroll 4
   for (int k = 0; k < kc; ++k) {
     const double2 a01 = *reinterpret_cast<const double2*>(pa + k * LD);
-    const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 64);
+    const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 16);
 #pragma unroll
     for (int t = 0; t < NTS; ++t) {
-      const double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * t);
-      acc[0][2 * t] = fma(a01.x, b.x, acc[0][2 * t]);
-      acc[0][2 * t + 1] = fma(a01.x, b.y, acc[0][2 * t + 1]);
-      acc[1][2 * t] = fma(a01.y, b.x, acc[1][2 * t]);
-      acc[1][2 * t + 1] = fma(a01.y, b.y, acc[1][2 * t + 1]);
-      acc[2][2 * t] = fma(a23.x, b.x, acc[2][2 * t]);
-      acc[2][2 * t + 1] = fma(a23.x, b.y, acc[2][2 * t + 1]);
-      acc[3][2 * t] = fma(a23.y, b.x, acc[3][2 * t]);
-      acc[3][2 * t + 1] = fma(a23.y, b.y, acc[3][2 * t + 1]);
+      if (t < rho::NTP_F) {
+        double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * t);
+        if (t == NTS - 1 && !last_ok) b = make_double2(0.0, 0.0);
+        rho_f_fma8(acc, t, a01, a23, b);
+      }
     }
   }
 }
 
-// The chunk's own columns [o0, o0 + kc) of the tile (o0 = 16 T0): this warp's pairs there are slots T0 and T0 + 1,
-// columns c = 16 t + 2 w; D'[k][c] = 0 for chunk rows k < c - o0, so the pair starts at k = c - o0.  After the chunk
-// these columns of X' are final and their Phi columns are the chunk's own columns c - o0 of the stage: epilogue.
+// The chunk's own columns [o0, o0 + kc) of the tile (o0 = 16 T0): an owner's pairs there are slots T0 and T0 + 1,
+// columns c = 16 t + 2 o.  D'[k][c] = 0 for chunk rows k < c - o0 (the stage holds those zeros), so every lane of the
+// warp may start at the warp's first row 16 tt + 8 wc.  After the chunk these columns of X' are final and their Phi
+// columns are the chunk's own columns c - o0 of the stage: epilogue.
 template <int T0>
 __device__ __forceinline__ void rho_f_diag(double (&acc)[4][2 * rho::NTP_F], double (&rs)[4],
-                                           const double* __restrict__ pa, const double* __restrict__ db, int kc, int w) {
+                                           const double* __restrict__ pa, const double* __restrict__ db, int kc, int wc,
+                                           int o) {
 #pragma unroll
   for (int tt = 0; tt < 2; ++tt) {
-    constexpr int dummy = 0;
-    (void)dummy;
-    const int t = T0 + tt;
     if (T0 + tt < rho::NTP_F) {
-      const int ks = 16 * tt + 2 * w;  // first chunk row that reaches this pair
-      if (ks < kc) {
-        for (int k = ks; k < kc; ++k) {
+      const int k_lo = 16 * tt + 8 * wc;   // warp-uniform
+      const int ks = 16 * tt + 2 * o;      // the lane's own first row = its pair's chunk column
+      const bool valid = ks < kc;          // beyond a ragged last chunk the stage columns are not written
+      if (k_lo < kc) {
+        for (int k = k_lo; k < kc; ++k) {
           const double2 a01 = *reinterpret_cast<const double2*>(pa + k * LD);
-          const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 64);
-          const double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * t);
-          acc[0][2 * (T0 + tt)] = fma(a01.x, b.x, acc[0][2 * (T0 + tt)]);
-          acc[0][2 * (T0 + tt) + 1] = fma(a01.x, b.y, acc[0][2 * (T0 + tt) + 1]);
-          acc[1][2 * (T0 + tt)] = fma(a01.y, b.x, acc[1][2 * (T0 + tt)]);
-          acc[1][2 * (T0 + tt) + 1] = fma(a01.y, b.y, acc[1][2 * (T0 + tt) + 1]);
-          acc[2][2 * (T0 + tt)] = fma(a23.x, b.x, acc[2][2 * (T0 + tt)]);
-          acc[2][2 * (T0 + tt) + 1] = fma(a23.x, b.y, acc[2][2 * (T0 + tt) + 1]);
-          acc[3][2 * (T0 + tt)] = fma(a23.y, b.x, acc[3][2 * (T0 + tt)]);
-          acc[3][2 * (T0 + tt) + 1] = fma(a23.y, b.y, acc[3][2 * (T0 + tt) + 1]);
+          const double2 a23 = *reinterpret_cast<const double2*>(pa + k * LD + 16);
+          double2 b = *reinterpret_cast<const double2*>(db + k * (rho::NT + 4) + 16 * (T0 + tt));
+          if (!valid) b = make_double2(0.0, 0.0);
+          rho_f_fma8(acc, T0 + tt, a01, a23, b);
         }
+        if (valid) {
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {  // epilogue: X'[rows][c + e] . Phi[rows][c + e], Phi column = chunk column ks + e
-          const double2 p01 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD);
-          const double2 p23 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD + 64);
-          rs[0] = fma(acc[0][2 * (T0 + tt) + e], p01.x, rs[0]);
-          rs[1] = fma(acc[1][2 * (T0 + tt) + e], p01.y, rs[1]);
-          rs[2] = fma(acc[2][2 * (T0 + tt) + e], p23.x, rs[2]);
-          rs[3] = fma(acc[3][2 * (T0 + tt) + e], p23.y, rs[3]);
+          for (int e = 0; e < 2; ++e) {  // epilogue: X'[rows][c + e] . Phi[rows][c + e], Phi column = chunk column ks + e
+            const double2 p01 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD);
+            const double2 p23 = *reinterpret_cast<const double2*>(pa + (ks + e) * LD + 16);
+            rs[0] = fma(acc[0][2 * (T0 + tt) + e], p01.x, rs[0]);
+            rs[1] = fma(acc[1][2 * (T0 + tt) + e], p01.y, rs[1]);
+            rs[2] = fma(acc[2][2 * (T0 + tt) + e], p23.x, rs[2]);
+            rs[3] = fma(acc[3][2 * (T0 + tt) + e], p23.y, rs[3]);
+          }
         }
       }
     }
@@ -226,6 +239,7 @@ __device__ __forceinline__ void rho_consumer_dfma(unsigned char* smem, const int
   double acc[4][2 * NTP_F];
   double rs[4] = {0.0, 0.0, 0.0, 0.0};
   double* red = reinterpret_cast<double*>(smem + RED_OFF);
+  const int wr = warp >> 1, wc = warp & 1, g = lane >> 2, h = lane & 3, o = 4 * wc + h;
   int s = 0;
   uint32_t ph = 0;
   for (;;) {
@@ -240,42 +254,45 @@ __device__ __forceinline__ void rho_consumer_dfma(unsigned char* smem, const int
 #pragma unroll
         for (int j = 0; j < 2 * NTP_F; ++j) acc[i][j] = 0.0;
     }
-    const double* pa = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * lane;            // rows of column k
-    const double* db = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + 2 * warp;  // pair slot 0
-    const int cw = ecnt ? o0 : wact;                                  // width of the rectangle before the own columns
-    const int nts = cw > 2 * warp ? (cw - 2 * warp + 15) >> 4 : 0;    // this warp's pair slots inside it
+    const double* pa = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 32 * wr + 2 * g;   // rows of column k
+    const double* db = reinterpret_cast<const double*>(smem + s * STAGE_BYTES + PHI_BYTES) + 2 * o;  // pair slot 0
+    const int cw = ecnt ? o0 : wact;                                   // width of the rectangle before the own columns
+    const int nts = cw > 8 * wc ? (cw - 8 * wc + 15) >> 4 : 0;         // pair slots of the warp's first owner (uniform)
+    const bool last_ok = 16 * (nts - 1) + 2 * o < cw;                  // this lane's last slot is inside the rectangle
     switch (nts) {
-      case 1: rho_f_rect<1>(acc, pa, db, kc); break;
-      case 2: rho_f_rect<2>(acc, pa, db, kc); break;
-      case 3: rho_f_rect<3>(acc, pa, db, kc); break;
-      case 4: rho_f_rect<4>(acc, pa, db, kc); break;
-      case 5: rho_f_rect<5>(acc, pa, db, kc); break;
-      case 6: rho_f_rect<6>(acc, pa, db, kc); break;
+      case 1: rho_f_rect<1>(acc, pa, db, kc, last_ok); break;
+      case 2: rho_f_rect<2>(acc, pa, db, kc, last_ok); break;
+      case 3: rho_f_rect<3>(acc, pa, db, kc, last_ok); break;
+      case 4: rho_f_rect<4>(acc, pa, db, kc, last_ok); break;
+      case 5: rho_f_rect<5>(acc, pa, db, kc, last_ok); break;
+      case 6: rho_f_rect<6>(acc, pa, db, kc, last_ok); break;
       default: break;
     }
     if (ecnt) {
       switch (o0 >> 5) {
-        case 0: rho_f_diag<0>(acc, rs, pa, db, kc, warp); break;
-        case 1: rho_f_diag<2>(acc, rs, pa, db, kc, warp); break;
-        default: rho_f_diag<4>(acc, rs, pa, db, kc, warp); break;
+        case 0: rho_f_diag<0>(acc, rs, pa, db, kc, wc, o); break;
+        case 1: rho_f_diag<2>(acc, rs, pa, db, kc, wc, o); break;
+        default: rho_f_diag<4>(acc, rs, pa, db, kc, wc, o); break;
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
     if (++s == NST) { s = 0; ph ^= 1; }
 
-    if (fl & F_LAST_PANEL) {  // rho_p: fixed-order sum of the 8 warps' partial row sums
-      *reinterpret_cast<double2*>(red + warp * GB + 2 * lane) = make_double2(rs[0], rs[1]);
-      *reinterpret_cast<double2*>(red + warp * GB + 64 + 2 * lane) = make_double2(rs[2], rs[3]);
+    if (fl & F_LAST_PANEL) {  // rho_p: the 4 owners of a warp by shuffle, the 2 column halves through shared memory
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        rs[i] += __shfl_xor_sync(0xffffffffu, rs[i], 1);
+        rs[i] += __shfl_xor_sync(0xffffffffu, rs[i], 2);
+      }
+      if (h == 0) {
+        *reinterpret_cast<double2*>(red + wc * GB + 32 * wr + 2 * g) = make_double2(rs[0], rs[1]);
+        *reinterpret_cast<double2*>(red + wc * GB + 32 * wr + 16 + 2 * g) = make_double2(rs[2], rs[3]);
+      }
       rs[0] = rs[1] = rs[2] = rs[3] = 0.0;
       asm volatile("bar.sync 2, %0;" ::"n"(32 * NCW_F) : "memory");
       const int r = warp * 32 + lane;
-      if (r < GB) {
-        double v = 0.0;
-#pragma unroll
-        for (int w2 = 0; w2 < NCW_F; ++w2) v += red[w2 * GB + r];
-        rho_s[(int64_t)p * GB + r] = 2.0 * v;
-      }
+      if (r < GB) rho_s[(int64_t)p * GB + r] = 2.0 * (red[r] + red[GB + r]);
       asm volatile("bar.sync 2, %0;" ::"n"(32 * NCW_F) : "memory");
     }
   }
