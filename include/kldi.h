@@ -204,7 +204,8 @@ kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, d
  * one pass over D and one over the retained-pair lists per call, pays off for a localised D.
  * KLDI_OPT_RHO_DFMA: 0 (default) = the LDA rho contraction runs on FP64 tensor-core DMMA tiles; 1 = on the vector FP64
  * pipe with register tiles (experimental and currently SLOWER, 6.1 vs 3.8 ms on cfg3: DMMA.8x8x4 tops out at 80 % of
- * the FP64 unit rate on B200 and DFMA does not, but this first version reaches 46 % of the pipe);
+ * the FP64 unit rate on B200 and DFMA does not, but register tiles that fit the register file are bound by the
+ * shared-memory wavefront rate);
  * same result to rounding, rho still bitwise reproducible; ignored while KLDI_OPT_PAIR_TEST is on and for GGA. */
 typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2, KLDI_OPT_RHO_DFMA = 3 } kldi_option;
 kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
