@@ -133,6 +133,23 @@ __device__ __forceinline__ void rho_epi_gga(const double (&acc)[16][2], double (
   }
 }
 
+// X-only epilogue (IMPL = 2, the X build of kldi_exc_grad): the stage holds 64 columns of Phi alone; column groups
+// J0..J0+7 of the finished X tile give rho and go to the X store.  Four times fewer epilogue stages than the GGA form,
+// and an epilogue stage costs one memory latency whatever it carries.
+template <int J0>
+__device__ __forceinline__ void rho_epi_x(const double (&acc)[16][2], double& rs, const double* __restrict__ es, int eb,
+                                          double* __restrict__ xg) {
+#pragma unroll
+  for (int jj = 0; jj < 8; ++jj) {
+    if (jj < eb) {
+      const double* e = es + jj * 8 * LD;
+      xg[(jj * 8) * GB] = acc[J0 + jj][0];
+      xg[(jj * 8 + 1) * GB] = acc[J0 + jj][1];
+      rs += acc[J0 + jj][0] * e[0] + acc[J0 + jj][1] * e[LD];
+    }
+  }
+}
+
 __device__ __forceinline__ void rho_stage(double (&acc)[16][2], const double* __restrict__ ps,
                                           const double* __restrict__ ds, int nks, int nj) {
   switch (nj) {
@@ -299,7 +316,7 @@ __device__ __forceinline__ void rho_consumer_dfma(unsigned char* smem, const int
 }
 
 template <bool GGA, bool TRI, int IMPL = 0>
-__global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTHREADS, 1)
+__global__ void __launch_bounds__(IMPL == 1 ? 32 * (rho::NCW_F + rho::NPW) : rho::NTHREADS, 1)
     k_rho(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket,
           const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off, const int32_t* __restrict__ colidx,
           const double* __restrict__ phi, const double* __restrict__ dphi0, const double* __restrict__ dphi1,
@@ -307,9 +324,11 @@ __global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTH
           double* __restrict__ drho_s, int64_t n_pad, const unsigned long long* __restrict__ pmask,
           double* __restrict__ x_store) {
   using namespace rho;
-  static_assert(IMPL == 0 || (TRI && !GGA), "the DFMA consumer implements the LDA (triangular) form");
-  constexpr int NCWI = IMPL ? NCW_F : NCW;  // consumer warps
-  constexpr int TW = IMPL ? TW_F : NT;      // N-tile width
+  static_assert(IMPL != 1 || (TRI && !GGA), "the DFMA consumer implements the LDA (triangular) form");
+  static_assert(IMPL != 2 || (GGA && !TRI), "the X-only epilogue belongs to the full-D form");
+  constexpr int NCWI = IMPL == 1 ? NCW_F : NCW;  // consumer warps
+  constexpr int TW = IMPL == 1 ? TW_F : NT;      // N-tile width
+  constexpr int ECI = IMPL == 2 ? 64 : EC;       // tile columns per epilogue stage
   extern __shared__ __align__(128) unsigned char smem[];
   int* hdr = reinterpret_cast<int*>(smem + NST * STAGE_BYTES);
   const uint32_t bar0 = smem_u32(smem + NST * STAGE_BYTES + NST * 16);  // full[s] at +8s, empty[s] at +8(NST+s)
@@ -406,9 +425,9 @@ __global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTH
           // epilogue operands through the ring: stage e holds columns [n0+16e, n0+16e+16) of the four stores,
           // producer warp a stages array a; the consumers contract them with the finished X tile from shared memory
           const double* arr = pw == 0 ? phi : pw == 1 ? dphi0 : pw == 2 ? dphi1 : dphi2;
-          const int nes = (Wj + EC - 1) / EC;
+          const int nes = (Wj + ECI - 1) / ECI;
           for (int e = 0; e < nes; ++e) {
-            const int ec = min(EC, Wj - EC * e);
+            const int ec = min(ECI, Wj - ECI * e);
             mbar_wait(bar0 + 8 * (NST + s), ph ^ 1);
             const uint32_t full = bar0 + 8 * s;
             if (pw == 0 && lane == 0) {
@@ -416,10 +435,14 @@ __global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTH
               hdr[4 * s + 1] = n0;
               hdr[4 * s + 2] = (F_EPI | ((e == nes - 1 && jt == ntile - 1) ? F_LAST_PANEL : 0)) << 16;
               hdr[4 * s + 3] = e | ((ec >> 3) << 8);
-              mbar_arrive_expect_tx(full, (uint32_t)(4 * ec) * (GB * 8));
+              mbar_arrive_expect_tx(full, (uint32_t)((IMPL == 2 ? 1 : 4) * ec) * (GB * 8));
             }
             __syncwarp();
-            if (lane < ec)
+            if (IMPL == 2) {  // Phi alone, 64 columns: producer warp pw copies columns 16 pw .. 16 pw + 15
+              if (lane < 16 && 16 * pw + lane < ec)
+                bulk_g2s(smem_u32(smem + s * STAGE_BYTES) + (16 * pw + lane) * (LD * 8),
+                         phi + (base + n0 + ECI * e + 16 * pw + lane) * GB, GB * 8, full);
+            } else if (lane < ec)
               bulk_g2s(smem_u32(smem + s * STAGE_BYTES) + (pw * EC + lane) * (LD * 8),
                        arr + (base + n0 + EC * e + lane) * GB, GB * 8, full);
             cp_async_mbar_arrive_noinc(full);
@@ -458,10 +481,16 @@ __global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTH
     const double* es = reinterpret_cast<const double*>(smem + s * STAGE_BYTES) + 2 * r4 * LD + 8 * warp + q4;
     if (GGA && (fl & F_EPI)) {
       if constexpr (GGA) {
-        const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2)
+        const int eb = h3 >> 8;  // 8-column groups in this stage (1 or 2; X-only form: up to 8)
         double* xg = nullptr;
         if (x_store)
-          xg = x_store + (panel_off[p] + hdr[4 * s + 1] + EC * (h3 & 0xff) + 2 * r4) * GB + 8 * warp + q4;
+          xg = x_store + (panel_off[p] + hdr[4 * s + 1] + ECI * (h3 & 0xff) + 2 * r4) * GB + 8 * warp + q4;
+        if constexpr (IMPL == 2) {
+          if ((h3 & 0xff) == 0)
+            rho_epi_x<0>(acc, rs[0], es, eb, xg);
+          else
+            rho_epi_x<8>(acc, rs[0], es, eb, xg);
+        } else
         switch (h3 & 0xff) {
 #define KLDI_CASE(E) case E: rho_epi_gga<2 * E>(acc, rs, es, eb, xg); break;
           KLDI_CASE(0) KLDI_CASE(1) KLDI_CASE(2) KLDI_CASE(3) KLDI_CASE(4) KLDI_CASE(5) KLDI_CASE(6) KLDI_CASE(7)
@@ -497,7 +526,7 @@ __global__ void __launch_bounds__(IMPL ? 32 * (rho::NCW_F + rho::NPW) : rho::NTH
 
     if (fl & F_LAST_PANEL) {  // rho_p (and grad rho_p) of this warp's 8 rows: quad reduction, one store per row
 #pragma unroll
-      for (int c = 0; c < (GGA ? 4 : 1); ++c) {
+      for (int c = 0; c < ((GGA && IMPL != 2) ? 4 : 1); ++c) {
         double v = rs[c];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
@@ -686,6 +715,7 @@ static kldi_status set_attrs() {
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES_F));
+  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
   g_attr_done = 1;
   return KLDI_OK;
 }
@@ -713,7 +743,11 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
     pm = P->d_pmask;
   }
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
-  if (gga)
+  if (gga && x_store)  // the X build of kldi_exc_grad: rho and the X store, no grad rho
+    k_rho<true, false, 2><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(
+        P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr, nullptr,
+        P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s, P->n_pad, pm, x_store);
+  else if (gga)
     k_rho<true, false><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off,
                                                            P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                                                            P->d_dphi[2], P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s,
