@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 #include <numeric>
 
 #include "ao_eval.cuh"
@@ -232,6 +233,85 @@ __global__ void __launch_bounds__(128) k_fill(ShellTable T, const int32_t* __res
   }
 }
 
+// --------------------------------------------------------------------------------- P5: BCS build on the device
+// The keep mask of the filter (Eq. 12) becomes BCS(R) by count -> prefix sum -> compaction (the mask + prefix-sum
+// pair selection of Alg. 1, applied to the block layout of PAPER.md:459-471), one warp per grid
+// block; BCS(C) is its transpose by a stable radix sort of the entries on their shell index.
+__global__ void __launch_bounds__(256) k_bcs_count(const uint8_t* __restrict__ keep, int n_shells,
+                                                   const int32_t* __restrict__ sh_ao0, int64_t n_blocks,
+                                                   int64_t* __restrict__ cnt, int32_t* __restrict__ kp,
+                                                   int64_t* __restrict__ k8) {
+  const int64_t p = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (p > n_blocks) return;
+  int c = 0, k = 0;
+  if (p < n_blocks)
+    for (int s = lane; s < n_shells; s += 32)
+      if (keep[p * n_shells + s]) {
+        c++;
+        k += sh_ao0[s + 1] - sh_ao0[s];
+      }
+  for (int o = 16; o > 0; o >>= 1) {
+    c += __shfl_xor_sync(0xffffffffu, c, o);
+    k += __shfl_xor_sync(0xffffffffu, k, o);
+  }
+  if (lane == 0) {  // entry n_blocks is the zero that turns the exclusive scans into [n_blocks + 1] offset arrays
+    cnt[p] = c;
+    k8[p] = (k + 7) & ~7;
+    if (p < n_blocks) kp[p] = k;
+  }
+}
+
+__global__ void k_narrow(const int64_t* __restrict__ in, int64_t n, int32_t* __restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (int32_t)in[i];
+}
+
+__global__ void __launch_bounds__(256) k_bcs_fill(const uint8_t* __restrict__ keep, int n_shells,
+                                                  const int32_t* __restrict__ sh_ao0, int64_t n_blocks,
+                                                  const int32_t* __restrict__ row_ptr,
+                                                  const int64_t* __restrict__ panel_off, const int32_t* __restrict__ kp,
+                                                  int32_t* __restrict__ col_idx, int32_t* __restrict__ blk_col0,
+                                                  int32_t* __restrict__ entry_row, int32_t* __restrict__ entry_id,
+                                                  int32_t* __restrict__ colidx, int32_t* __restrict__ col_cnt) {
+  const int64_t p = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (p >= n_blocks) return;
+  int e_base = row_ptr[p], kbase = 0;
+  const int64_t base = panel_off[p];
+  for (int s0 = 0; s0 < n_shells; s0 += 32) {
+    const int s = s0 + lane;
+    const bool kept = s < n_shells && keep[p * n_shells + s];
+    const int w = kept ? sh_ao0[s + 1] - sh_ao0[s] : 0;
+    const unsigned m = __ballot_sync(0xffffffffu, kept);
+    int incl = w;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (kept) {
+      const int e = e_base + __popc(m & ((1u << lane) - 1u));
+      const int k0 = kbase + incl - w;
+      col_idx[e] = s;
+      blk_col0[e] = k0;
+      entry_row[e] = (int32_t)p;
+      entry_id[e] = e;
+      atomicAdd(col_cnt + s + 1, 1);
+      for (int c = 0; c < w; ++c) colidx[base + k0 + c] = sh_ao0[s] + c;
+    }
+    e_base += __popc(m);
+    kbase += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  const int k = kp[p], k8 = (k + 7) & ~7;
+  for (int c = k + lane; c < k8; c += 32) colidx[base + c] = 0;  // zero columns: any valid AO index
+}
+
+__global__ void k_gather_i32(const int32_t* __restrict__ src, const int32_t* __restrict__ idx, int64_t n,
+                             int32_t* __restrict__ dst) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = src[idx[i]];
+}
+
 // --------------------------------------------------------------------------------- host helpers
 template <class T>
 static kldi_status upload(T** dst, const std::vector<T>& v, cudaStream_t st, size_t extra = 0) {
@@ -370,9 +450,12 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   int32_t* d_idx_in = nullptr;
   void* d_tmp = nullptr;
   uint8_t* d_keep = nullptr;
+  int64_t *d_cnt64 = nullptr, *d_k8 = nullptr, *d_rp64 = nullptr;
+  int32_t *d_erow = nullptr, *d_eid = nullptr, *d_skey = nullptr, *d_ccnt = nullptr;
   auto cleanup = [&]() {
     cudaFree(d_atom_sh0); cudaFree(d_xyz); cudaFree(d_w); cudaFree(d_keys_in); cudaFree(d_idx_in);
     cudaFree(d_tmp); cudaFree(d_keep);
+    cudaFree(d_cnt64); cudaFree(d_k8); cudaFree(d_rp64); cudaFree(d_erow); cudaFree(d_eid); cudaFree(d_skey); cudaFree(d_ccnt);
   };
 #define CK(call)                        \
   do {                                  \
@@ -417,44 +500,111 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
     k_screen<false><<<(int)n_blocks, 128, 0, st>>>(T, d_atom_sh0, n_atoms, n_shells, P->d_gx, P->d_gy, P->d_gz,
                                                    P->eps, d_keep);
   CK(cudaGetLastError());
-  std::vector<uint8_t> h_keep(mask_bytes);
-  CK(cudaMemcpyAsync(h_keep.data(), d_keep, mask_bytes, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-
-  // ---- P5: BCS(R), packed column maps, BCS(C)
+  // ---- P5: BCS(R), packed column maps, BCS(C) — built on the device, host copies kept for export / statistics
   auto& row_ptr = P->h_row_ptr;
   auto& col_idx = P->h_col_idx;
   auto& blk_col0 = P->h_blk_col0;
   auto& panel_off = P->h_panel_off;
+  auto& col_ptr = P->h_col_ptr;
+  auto& row_idx = P->h_row_idx;
+  auto& pos = P->h_pos;
+  std::vector<int32_t> h_kp(n_blocks), h_tasks;
+  const int nbw = (int)((n_blocks + 1 + 7) / 8);
+  CK(cudaMalloc(&d_cnt64, sizeof(int64_t) * (n_blocks + 1)));
+  CK(cudaMalloc(&d_k8, sizeof(int64_t) * (n_blocks + 1)));
+  CK(cudaMalloc(&d_rp64, sizeof(int64_t) * (n_blocks + 1)));
+  CK(cudaMalloc(&P->d_kp, sizeof(int32_t) * std::max<int64_t>(1, n_blocks)));
+  CK(cudaMalloc(&P->d_panel_off, sizeof(int64_t) * (n_blocks + 1)));
+  CK(cudaMalloc(&P->d_row_ptr, sizeof(int32_t) * (n_blocks + 1)));
+  k_bcs_count<<<nbw, 256, 0, st>>>(d_keep, n_shells, P->d_sh_ao0, n_blocks, d_cnt64, P->d_kp, d_k8);
+  CK(cudaGetLastError());
+  {
+    size_t need = 0;
+    CK(cub::DeviceScan::ExclusiveSum(nullptr, need, d_cnt64, d_rp64, (int)(n_blocks + 1), st));
+    if (need > tmp_bytes) {
+      cudaFree(d_tmp);
+      d_tmp = nullptr;
+      CK(cudaMalloc(&d_tmp, need));
+      tmp_bytes = need;
+    }
+    CK(cub::DeviceScan::ExclusiveSum(d_tmp, tmp_bytes, d_cnt64, d_rp64, (int)(n_blocks + 1), st));
+    CK(cub::DeviceScan::ExclusiveSum(d_tmp, tmp_bytes, d_k8, P->d_panel_off, (int)(n_blocks + 1), st));
+  }
+  int64_t retained = 0;
+  CK(cudaMemcpyAsync(&retained, d_rp64 + n_blocks, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(&P->total_cols, P->d_panel_off + n_blocks, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (retained >= ((int64_t)1 << 31) - 4096) {
+    set_error("too many retained blocks for int32 BCS indices");
+    cleanup();
+    return KLDI_EINVAL;
+  }
+  k_narrow<<<(int)((n_blocks + 1 + 255) / 256), 256, 0, st>>>(d_rp64, n_blocks + 1, P->d_row_ptr);
+  CK(cudaGetLastError());
+  const int64_t r1 = std::max<int64_t>(1, retained);
+  CK(cudaMalloc(&P->d_col_idx, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&P->d_blk_col0, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&P->d_row_idx, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&P->d_pos, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&d_erow, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&d_eid, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&d_skey, sizeof(int32_t) * r1));
+  CK(cudaMalloc(&P->d_colidx, sizeof(int32_t) * std::max<int64_t>(1, P->total_cols)));
+  CK(cudaMalloc(&P->d_col_ptr, sizeof(int32_t) * (n_shells + 1)));
+  CK(cudaMalloc(&d_ccnt, sizeof(int32_t) * (n_shells + 1)));
+  CK(cudaMemsetAsync(d_ccnt, 0, sizeof(int32_t) * (n_shells + 1), st));
+  k_bcs_fill<<<(int)((n_blocks + 7) / 8), 256, 0, st>>>(d_keep, n_shells, P->d_sh_ao0, n_blocks, P->d_row_ptr,
+                                                       P->d_panel_off, P->d_kp, P->d_col_idx, P->d_blk_col0, d_erow,
+                                                       d_eid, P->d_colidx, d_ccnt);
+  CK(cudaGetLastError());
+  {  // BCS(C): col_ptr = inclusive scan of the per-shell counts; entries stably sorted by shell (ascending p inside)
+    size_t need = 0;
+    CK(cub::DeviceScan::InclusiveSum(nullptr, need, d_ccnt, P->d_col_ptr, n_shells + 1, st));
+    size_t need2 = 0;
+    int bits = 1;
+    while ((1 << bits) < n_shells) ++bits;
+    if (retained > 0)
+      CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, P->d_col_idx, d_skey, d_eid, P->d_pos, (int)retained, 0, bits,
+                                         st));
+    need = std::max(need, need2);
+    if (need > tmp_bytes) {
+      cudaFree(d_tmp);
+      d_tmp = nullptr;
+      CK(cudaMalloc(&d_tmp, need));
+      tmp_bytes = need;
+    }
+    CK(cub::DeviceScan::InclusiveSum(d_tmp, tmp_bytes, d_ccnt, P->d_col_ptr, n_shells + 1, st));
+    if (retained > 0) {
+      CK(cub::DeviceRadixSort::SortPairs(d_tmp, tmp_bytes, P->d_col_idx, d_skey, d_eid, P->d_pos, (int)retained, 0,
+                                         bits, st));
+      k_gather_i32<<<(int)((retained + 255) / 256), 256, 0, st>>>(d_erow, P->d_pos, retained, P->d_row_idx);
+      CK(cudaGetLastError());
+    }
+  }
+  // host copies (export, statistics, task list, V schedule)
   row_ptr.assign(n_blocks + 1, 0);
   panel_off.assign(n_blocks + 1, 0);
-  col_idx.clear();
-  blk_col0.clear();
-  std::vector<int32_t> h_kp(n_blocks), h_colidx, h_tasks;
-  std::vector<int32_t> col_cnt(n_shells + 1, 0);
+  col_idx.assign(retained, 0);
+  blk_col0.assign(retained, 0);
+  row_idx.assign(retained, 0);
+  pos.assign(retained, 0);
+  col_ptr.assign(n_shells + 1, 0);
+#define DH(vec, dptr) \
+  if (!(vec).empty()) CK(cudaMemcpyAsync((vec).data(), (dptr), (vec).size() * sizeof((vec)[0]), cudaMemcpyDeviceToHost, st))
+  DH(row_ptr, P->d_row_ptr);
+  DH(panel_off, P->d_panel_off);
+  DH(col_idx, P->d_col_idx);
+  DH(blk_col0, P->d_blk_col0);
+  DH(row_idx, P->d_row_idx);
+  DH(pos, P->d_pos);
+  DH(col_ptr, P->d_col_ptr);
+  DH(h_kp, P->d_kp);
+#undef DH
+  CK(cudaStreamSynchronize(st));
   double f_rho_u = 0, f_v_u = 0, f_rho_us = 0;
   int64_t sum_k = 0, max_k = 0;
   for (int64_t p = 0; p < n_blocks; ++p) {
-    const uint8_t* kp = h_keep.data() + (size_t)p * n_shells;
-    int k = 0;
-    for (int s = 0; s < n_shells; ++s)
-      if (kp[s]) {
-        col_idx.push_back(s);
-        blk_col0.push_back(k);
-        col_cnt[s + 1]++;
-        for (int c = h_sh_ao0[s]; c < h_sh_ao0[s + 1]; ++c) h_colidx.push_back(c);
-        k += h_sh_ao0[s + 1] - h_sh_ao0[s];
-      }
-    if (col_idx.size() >= ((size_t)1 << 31) - 4096) {
-      set_error("too many retained blocks for int32 BCS indices");
-      cleanup();
-      return KLDI_EINVAL;
-    }
-    const int k8 = (k + 7) & ~7;
-    for (int c = k; c < k8; ++c) h_colidx.push_back(0);  // zero columns: any valid AO index
-    h_kp[p] = k;
-    row_ptr[p + 1] = (int32_t)col_idx.size();
-    panel_off[p + 1] = panel_off[p] + k8;
+    const int k = h_kp[p];
     if (k > 0) h_tasks.push_back((int32_t)p);
     sum_k += k;
     max_k = std::max<int64_t>(max_k, k);
@@ -462,37 +612,6 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
     f_rho_us += (double)GB * k * (k + 1.0);
     f_v_u += P->want_grad ? 2.0 * GB * (double)k * k : (double)GB * k * (k + 1.0);
   }
-  P->total_cols = panel_off[n_blocks];
-  const int64_t retained = (int64_t)col_idx.size();
-  // BCS(C): for every AO block the grid blocks that retain it, and where
-  auto& col_ptr = P->h_col_ptr;
-  auto& row_idx = P->h_row_idx;
-  auto& pos = P->h_pos;
-  col_ptr.assign(n_shells + 1, 0);
-  for (int s = 0; s < n_shells; ++s) col_ptr[s + 1] = col_ptr[s] + col_cnt[s + 1];
-  row_idx.assign(retained, 0);
-  pos.assign(retained, 0);
-  {
-    std::vector<int32_t> cur(col_ptr.begin(), col_ptr.end() - 1);
-    for (int64_t p = 0; p < n_blocks; ++p)
-      for (int32_t e = row_ptr[p]; e < row_ptr[p + 1]; ++e) {
-        const int32_t c = cur[col_idx[e]]++;
-        row_idx[c] = (int32_t)p;
-        pos[c] = e;
-      }
-  }
-  h_keep.clear();
-  h_keep.shrink_to_fit();
-
-  UP(P->d_row_ptr, row_ptr);
-  UP(P->d_col_idx, col_idx);
-  UP(P->d_blk_col0, blk_col0);
-  UP(P->d_col_ptr, col_ptr);
-  UP(P->d_row_idx, row_idx);
-  UP(P->d_pos, pos);
-  UP(P->d_panel_off, panel_off);
-  UP(P->d_kp, h_kp);
-  UP(P->d_colidx, h_colidx);
   // S: cost-sorted pull order.  Heavy grid blocks first so that the tail of the persistent kernels is made of light
   // ones; buckets of 96 columns, Morton order kept inside a bucket for the L2 locality of the D gather (measured:
   // cfg1 +2 %, cfg2 +1 %, cfg3 +0.3 % over plain Morton order; fully sorted by K_p loses the locality again).
