@@ -226,6 +226,8 @@ def becke_weights(atom_xyz: np.ndarray, pts: np.ndarray, owner: np.ndarray,
     if backend == "cuda":
         from . import becke_cuda
         return becke_cuda.becke_partition(atom_xyz, pts, owner)
+    if backend == "none":   # the caller supplies the final weights (named_config(grid_w=...))
+        return np.ones(pts.shape[0])
     return _becke_numpy(atom_xyz, pts, owner)
 
 
@@ -274,9 +276,12 @@ _CONFIGS = {
 
 
 def named_config(name: str, *, n_override: Optional[int] = None, functional: Optional[str] = None,
-                 eps: Optional[float] = None, cache: Optional[bool] = None, becke_backend: str = "auto") -> Workload:
+                 eps: Optional[float] = None, cache: Optional[bool] = None, becke_backend: str = "auto",
+                 grid_w: Optional[np.ndarray] = None) -> Workload:
     """BASELINE.json configs[0..4] as "cfg0".."cfg4".  `n_override` shrinks the molecule count
-    (waters or carbons) for reduced-size parity cases; same recipe, same seed."""
+    (waters or carbons) for reduced-size parity cases; same recipe, same seed.  `grid_w`: final quadrature
+    weights of this very config written earlier by this generator (e.g. with the CUDA Becke helper on a GPU box);
+    the Becke step is then skipped — for CPU-only runs of the large configs."""
     kind, size, fn, e, seed = _CONFIGS[name]
     if cache is None:
         cache = os.environ.get("KLDI_WL_CACHE", "0") == "1"
@@ -301,7 +306,13 @@ def named_config(name: str, *, n_override: Optional[int] = None, functional: Opt
     else:
         symbols, xyz = alkane_geometry(size)
         n_occ = (6 * size + (2 * size + 2)) // 2
-    wl = make_workload(tag, symbols, xyz, n_occ, fn, e, seed, becke_backend)
+    wl = make_workload(tag, symbols, xyz, n_occ, fn, e, seed, "none" if grid_w is not None else becke_backend)
+    if grid_w is not None:
+        grid_w = np.ascontiguousarray(grid_w, dtype=np.float64)
+        if grid_w.shape != wl.grid_w.shape:
+            raise ValueError(f"grid_w has shape {grid_w.shape}, config needs {wl.grid_w.shape}")
+        wl.grid_w = grid_w
+        return wl
     if cache and wl.n_pts >= 200_000:
         try:
             os.makedirs(cache_dir, exist_ok=True)
