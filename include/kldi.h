@@ -206,8 +206,16 @@ kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, d
  * pipe with register tiles (experimental and currently SLOWER, 6.1 vs 3.8 ms on cfg3: DMMA.8x8x4 tops out at 80 % of
  * the FP64 unit rate on B200 and DFMA does not, but register tiles that fit the register file are bound by the
  * shared-memory wavefront rate);
- * same result to rounding, rho still bitwise reproducible; ignored while KLDI_OPT_PAIR_TEST is on and for GGA. */
-typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2, KLDI_OPT_RHO_DFMA = 3 } kldi_option;
+ * same result to rounding, rho still bitwise reproducible; ignored while KLDI_OPT_PAIR_TEST is on and for GGA.
+ * KLDI_OPT_RHO_TC: 0 (default) = FP64 DMMA tiles; 1 = the LDA rho contraction runs as int8 slice products on the
+ * 5th-generation tensor cores (tcgen05.mma kind::i8, int32 accumulators in tensor memory, the paper's
+ * low-precision Tensor-Core multiplier, with error compensation): Phi (row scale, at first
+ * use) and D' (column scale, per call) are split into five signed base-256 digits, the 15 digit products of weight
+ * >= 256^-6 are accumulated exactly, and rho is recombined in FP64.  Error ~1e-10 absolute on rho (same parity bar,
+ * 1e-9); rho stays bitwise reproducible.  Costs a second store of 5 bytes per retained Phi value and n_ao^2 64-bit
+ * words.  Ignored for GGA, while KLDI_OPT_PAIR_TEST is on, and by kldi_eval_tau / kldi_exc_grad; KLDI_ESTATE from the
+ * compute call if a grid block retains more than 16384 AO columns. */
+typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2, KLDI_OPT_RHO_DFMA = 3, KLDI_OPT_RHO_TC = 4 } kldi_option;
 kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
 
 /* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`

@@ -27,6 +27,7 @@ EXPORTED = [
 KLDI_OPT_DETERMINISTIC_V = 1
 KLDI_OPT_PAIR_TEST = 2
 KLDI_OPT_RHO_DFMA = 3
+KLDI_OPT_RHO_TC = 4
 
 
 class KldiError(RuntimeError):

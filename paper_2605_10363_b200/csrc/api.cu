@@ -374,7 +374,8 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
 }
 
 kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
-  if (!P || (option != KLDI_OPT_DETERMINISTIC_V && option != KLDI_OPT_PAIR_TEST && option != KLDI_OPT_RHO_DFMA)) {
+  if (!P || (option != KLDI_OPT_DETERMINISTIC_V && option != KLDI_OPT_PAIR_TEST && option != KLDI_OPT_RHO_DFMA &&
+             option != KLDI_OPT_RHO_TC)) {
     set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);
     return KLDI_EINVAL;
   }
@@ -386,6 +387,7 @@ kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
     P->v_mode = value;
   }
   if (option == KLDI_OPT_RHO_DFMA) P->rho_impl = value ? 1 : 0;
+  if (option == KLDI_OPT_RHO_TC) P->rho_impl = value ? 2 : 0;
   if (option == KLDI_OPT_PAIR_TEST) {
     P->pair_test = value ? 1 : 0;
     if (!value) P->pair_counts_valid = false;

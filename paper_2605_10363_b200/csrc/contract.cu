@@ -733,6 +733,7 @@ kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
 kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
   kldi_status rc = set_attrs();
   if (rc != KLDI_OK) return rc;
+  if (!gga && P->rho_impl == 2 && !P->pair_test) return launch_rho_tc(P);
   KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
   if (gga) KLDI_CUDA(cudaMemsetAsync(P->d_drho_s, 0, sizeof(double) * 3 * P->n_pad, P->stream));
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));

@@ -97,7 +97,15 @@ struct kldi_plan {
   double* d_gram = nullptr;                       // lazily allocated workspace of G_p partials
   int64_t gram_cap = 0;
   int32_t* d_ao_shell = nullptr;                  // plan AO -> plan shell
-  int rho_impl = 0;                               // LDA rho build: 0 DMMA tiles, 1 DFMA register tiles (KLDI_OPT_RHO_DFMA)
+  int rho_impl = 0;                               // LDA rho build: 0 DMMA tiles, 1 DFMA register tiles (KLDI_OPT_RHO_DFMA),
+                                                  // 2 int8 slice products on tcgen05 (KLDI_OPT_RHO_TC)
+  // ---- int8 slice-product path (rho_i8.cu), allocated on first use
+  unsigned char* d_phiq = nullptr;                // [tc_chunks][NSL][4096] digit planes of Phi, tensor-core smem image
+  double* d_sigma = nullptr;                      // [n_pad] row scales of the digit planes
+  unsigned long long* d_Dq = nullptr;             // [n_ao][n_ao] packed digits of D' (per call)
+  double* d_tau = nullptr;                        // [2][n_ao] column scales of D', column maxima
+  int64_t* d_chunk_off = nullptr;                 // [n_blocks+1] first 32-column chunk of grid block p
+  int64_t tc_chunks = 0;
   int v_mode = 0;                                 // 0: red.global.add.f64 epilogue, 1: workspace + fixed-order reduce,
                                                   // 2: 64-bit fixed-point integer atomics (reproducible)
   double* d_fx = nullptr;                         // [1 + n_blocks] fixed-point bound, then s_p = sum_g |wv_g| per block
@@ -138,6 +146,8 @@ kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
 // pairsel.cu
 kldi_status launch_pair_select(kldi_plan* P, bool tri);
 kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store = nullptr);
+// rho_i8.cu
+kldi_status launch_rho_tc(kldi_plan* P);
 kldi_status launch_grad_cols(kldi_plan* P, double* grad);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);

@@ -1,0 +1,444 @@
+// H2 on the 5th-generation tensor cores: the LDA rho contraction as int8 slice products with exact int32
+// accumulation in tensor memory (the paper's low-precision Tensor-Core block multiplier,
+// PAPER.md:218-226, 499-501 App. A-E, with error compensation).  sm_100a: tcgen05.mma kind::i8 (SASS UTCIMMA),
+// TMEM accumulators, operands in shared memory, mbarrier pipeline.  KLDI_OPT_RHO_TC.
+//
+// Arithmetic.  Per grid block p with packed retained columns L(p):
+//     X' = Phi_p D'[L,L],  rho = 2 rowsum(Phi_p o X')        D' = lower triangle of D, diagonal halved
+// Both operands are split into NSL signed 8-bit digits of base 256 (an error-free transformation of the value rounded
+// to 8 NSL bits below its scale):
+//     Phi(g,k) ~ sigma_g  sum_i a_i(g,k) 256^-(i+1),   sigma_g = max_k |Phi(g,k)| * 256/127   (row scale, plan time)
+//     D'(k,n)  ~ tau_n    sum_j b_j(k,n) 256^-(j+1),   tau_n   = max_k |D'(k,n)|  * 256/127   (column scale, per call)
+// The digit pairs of equal weight c = i + j accumulate exactly in one int32 TMEM accumulator (|sum| <= K (c+1) 127^2 <
+// 2^31 for K <= 16384), classes c <= NSL-1 are kept (the dropped ones are below 256^-(NSL+1) relative to sigma tau K):
+//     X'(g,n) = sigma_g tau_n 256^-(NSL+1)  sum_c acc_c(g,n) 256^(NSL-1-c)
+// and the epilogue forms rho in FP64 from the int64 recombination and the FP64 Phi store.  NSL = 5: 15 int8 products,
+// max|d rho| ~ 1e-10 on the 8-water case (tolerance 1e-9); NSL = 6: 21 products, ~3e-13.
+#include <cstdio>
+
+#include "kldi_internal.h"
+#include "ptx.cuh"
+
+namespace kldi {
+namespace tc {
+
+constexpr int KC = 32;                       // K per tcgen05.mma kind::i8 = packed columns per ring stage
+constexpr int NT = 96;                       // N-tile width (NSL * NT <= 512 TMEM columns for NSL = 5)
+constexpr int A_SLICE = GB * KC;             // 4096 B: one digit plane of a 128 x 32 Phi chunk
+constexpr int NCH = NT / 16;                 // 16-column pieces of the B tile = gather warps per group
+constexpr int B_SLICE = NCH * 512;           // 3072 B: one digit plane of a 32 x 96 D' tile
+constexpr int NST = 4;                       // ring stages
+constexpr int NGRP = 2;                      // gather groups (alternate stages)
+constexpr int W_PROD = 0, W_MMA = 1, W_TMEM = 2, W_GATHER0 = 4, W_EPI0 = W_GATHER0 + NGRP * NCH;  // warp roles
+constexpr int NWARPS = W_EPI0 + 4;
+constexpr int NTHREADS = 32 * NWARPS;        // 640
+enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
+
+template <int NSL>
+struct Cfg {
+  static constexpr int STAGE_BYTES = NSL * (A_SLICE + B_SLICE);
+  static constexpr int OFF_HDR = NST * STAGE_BYTES;          // [NST][4] int
+  static constexpr int OFF_BAR = OFF_HDR + NST * 16;         // hdr_full[NST], full_a[NST], full_b[NST], empty[NST], tmem_full, tmem_empty
+  static constexpr int OFF_TMEM = OFF_BAR + (4 * NST + 2) * 8;
+  static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;  // [4 epilogue warps][NT] double
+  static constexpr int SMEM_BYTES = OFF_TAU + 4 * NT * 8;
+  static constexpr int TMEM_COLS = 512;
+  static_assert(NSL * NT <= 512, "accumulator classes do not fit tensor memory");
+};
+
+// byte offset of (row m of 128 | column n of the tile, k of the chunk) inside one MN-major digit plane
+__host__ __device__ __forceinline__ int plane_off(int mn, int k) {
+  return (mn >> 4) * 512 + (k >> 3) * 128 + (k & 7) * 16 + (mn & 15);
+}
+
+// ------------------------------------------------------------------------------------------------ plan side
+// Digit planes of Phi: per grid block the row scales sigma_g, then for every chunk of 32 packed columns NSL planes of
+// 4 KB in the shared-memory image the tensor core reads (so that a ring stage is ONE bulk copy).
+template <int NSL>
+__global__ void __launch_bounds__(128) k_slice_phi(const int32_t* __restrict__ tasks, const int32_t* __restrict__ kp,
+                                                   const int64_t* __restrict__ panel_off,
+                                                   const int64_t* __restrict__ chunk_off, const double* __restrict__ phi,
+                                                   double* __restrict__ sigma, unsigned char* __restrict__ phiq) {
+  __shared__ __align__(16) unsigned char tile[NSL * A_SLICE];
+  const int p = tasks[blockIdx.x], g = threadIdx.x;
+  const int K8 = (kp[p] + 7) & ~7;
+  const int64_t base = panel_off[p];
+  double mx = 0.0;
+  for (int k = 0; k < K8; ++k) mx = fmax(mx, fabs(phi[(base + k) * GB + g]));
+  const double sg = mx > 0.0 ? mx * (256.0 / 127.0) : 1.0;
+  sigma[(int64_t)p * GB + g] = sg;
+  const double inv = scalbn(1.0 / sg, 8 * NSL);
+  const int nchunk = (K8 + KC - 1) / KC;
+  for (int c = 0; c < nchunk; ++c) {
+    for (int kk = 0; kk < KC; ++kk) {
+      const int k = c * KC + kk;
+      long long n = 0;
+      if (k < K8) n = __double2ll_rn(phi[(base + k) * GB + g] * inv);
+#pragma unroll
+      for (int i = NSL - 1; i >= 0; --i) {  // balanced base-256 digits, least significant first
+        const int d = (int)(signed char)(n & 0xff);
+        tile[i * A_SLICE + plane_off(g, kk)] = (unsigned char)d;
+        n = (n - d) >> 8;
+      }
+    }
+    __syncthreads();
+    uint4* dst = reinterpret_cast<uint4*>(phiq + (chunk_off[p] + c) * (int64_t)(NSL * A_SLICE));
+    const uint4* src = reinterpret_cast<const uint4*>(tile);
+    for (int i = threadIdx.x; i < NSL * A_SLICE / 16; i += 128) dst[i] = src[i];
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ per call
+// tau_n = max_k |D'(k,n)| * 256/127 over the stored (lower-triangular, plan-order) D'.  Non-negative doubles order like
+// their bit patterns, so the column maximum is an integer atomicMax.
+__global__ void __launch_bounds__(256) k_colmax(const double* __restrict__ Dp, int n, unsigned long long* __restrict__ mx) {
+  const int j = blockIdx.x * 32 + (threadIdx.x & 31);
+  const int r0 = blockIdx.y * 256 + (threadIdx.x >> 5);
+  if (j >= n) return;
+  double m = 0.0;
+  for (int r = r0; r < min(n, blockIdx.y * 256 + 256); r += 8) m = fmax(m, fabs(Dp[(int64_t)r * n + j]));
+  if (m > 0.0) atomicMax(mx + j, (unsigned long long)__double_as_longlong(m));
+}
+
+// Dq[k][n] = the NSL digits of D'(k,n) / tau_n packed in one 64-bit word (byte i = digit i, most significant first);
+// tau[n] is rewritten in place from the maximum to the scale.
+template <int NSL>
+__global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, int n, const double* __restrict__ cmax,
+                                                 double* __restrict__ tau, unsigned long long* __restrict__ Dq) {
+  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y;
+  if (j >= n) return;
+  const double m = cmax[j];
+  const double t = m > 0.0 ? m * (256.0 / 127.0) : 1.0;
+  if (i == 0) tau[j] = t;
+  unsigned long long q = 0;
+  if (j <= i) {
+    long long v = __double2ll_rn(Dp[(int64_t)i * n + j] * scalbn(1.0 / t, 8 * NSL));
+#pragma unroll
+    for (int s = NSL - 1; s >= 0; --s) {
+      const int d = (int)(signed char)(v & 0xff);
+      q |= (unsigned long long)(unsigned char)d << (8 * s);
+      v = (v - d) >> 8;
+    }
+  }
+  Dq[(int64_t)i * n + j] = q;
+}
+
+// ------------------------------------------------------------------------------------------------ the contraction
+// Persistent, one CTA per SM, warp-specialised:
+//   warp 0      scheduler + A producer: pulls grid blocks from the atomic ticket, walks the block's
+//               (N-tile, K-chunk) stages, writes the stage header and bulk-copies the chunk's NSL digit planes of Phi
+//   warps 4-15  B builders, two groups of six on alternate stages: warp c of a group gathers the 16 columns
+//               [n0+16c, n0+16c+16) x 32 rows of D' (lane = K row, 16 x 8-byte digit words), transposes the bytes to
+//               digit planes with PRMT and stores them in the MN-major core-matrix layout (5 x 16-byte stores)
+//   warp 1      MMA issuer: one elected lane issues the NSL(NSL+1)/2 tcgen05.mma of a stage (A_i x B_j -> class i+j)
+//               and commits them to the stage's empty barrier (and to tmem_full after the last chunk of a tile)
+//   warps 16-19 epilogue: TMEM -> registers (one lane = one grid row), int64 recombination of the classes, FP64
+//               rho += tau_n Phi(g,n) X_int(g,n) with Phi from the FP64 store; rho_p at the end of the panel
+template <int NSL>
+__global__ void __launch_bounds__(NTHREADS, 1)
+    k_rho_i8(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket, const int32_t* __restrict__ kp,
+             const int64_t* __restrict__ panel_off, const int64_t* __restrict__ chunk_off,
+             const int32_t* __restrict__ colidx, const double* __restrict__ phi, const unsigned char* __restrict__ phiq,
+             const double* __restrict__ sigma, const unsigned long long* __restrict__ Dq, const double* __restrict__ tau,
+             int n_ao, double* __restrict__ rho_s) {
+  using C = Cfg<NSL>;
+  extern __shared__ __align__(128) unsigned char smem[];
+  volatile int* hdr = reinterpret_cast<volatile int*>(smem + C::OFF_HDR);
+  const uint32_t bar0 = smem_u32(smem + C::OFF_BAR);
+  const uint32_t b_hdr = bar0, b_fa = bar0 + 8 * NST, b_fb = bar0 + 16 * NST, b_empty = bar0 + 24 * NST;
+  const uint32_t b_tfull = bar0 + 32 * NST, b_tempty = b_tfull + 8;
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + C::OFF_TMEM);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(b_hdr + 8 * s, 1);
+      mbar_init(b_fa + 8 * s, 1);
+      mbar_init(b_fb + 8 * s, NCH);
+      mbar_init(b_empty + 8 * s, 1 + 4);  // tcgen05.commit of the stage's MMAs + the 4 epilogue warps (header read)
+    }
+    mbar_init(b_tfull, 1);
+    mbar_init(b_tempty, 4);
+    fence_mbar_init();
+  }
+  if (warp == W_TMEM) tmem_alloc(smem_u32(smem + C::OFF_TMEM), C::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == W_PROD) {
+    // ------------------------------------------------------------------ scheduler + A producer
+    uint32_t t = 0;  // stage sequence number: slot t % NST, use t / NST
+    auto acquire = [&](int s) {
+      if (t >= NST) mbar_wait(b_empty + 8 * s, ((t / NST) - 1) & 1);
+    };
+    for (;;) {
+      int task = 0;
+      if (lane == 0) task = atomicAdd(ticket, 1);
+      task = __shfl_sync(0xffffffffu, task, 0);
+      if (task >= n_tasks) break;
+      const int p = tasks[task];
+      const int K8 = (kp[p] + 7) & ~7, K32 = (K8 + KC - 1) & ~(KC - 1);
+      const int64_t cbase = chunk_off[p];
+      const int ntile = (K32 + NT - 1) / NT;
+      const int W = ((K32 / KC + ntile - 1) / ntile) * KC;  // tiles start on chunk boundaries
+      for (int jt = 0; jt < ntile; ++jt) {
+        const int n0 = jt * W, Wj = min(W, K32 - n0);
+        // D' is lower triangular in packed order: only the chunks k0 >= n0 reach this tile, and chunk [k0, k0+32)
+        // only its columns n < k0 + 32
+        for (int k0 = n0; k0 < K32; k0 += KC) {
+          const int s = t % NST;
+          acquire(s);
+          if (lane == 0) {
+            int fl = 0;
+            if (k0 == n0) fl |= F_FIRST;
+            if (k0 + KC >= K32) fl |= F_LAST_TILE | (jt == ntile - 1 ? F_LAST_PANEL : 0);
+            // the first chunk of a tile runs at full width: it overwrites (zeroes) every accumulator column of the tile
+            const int wact = k0 == n0 ? Wj : min(Wj, k0 + KC - n0);
+            hdr[4 * s + 0] = p;
+            hdr[4 * s + 1] = n0 | (k0 << 16);
+            hdr[4 * s + 2] = fl | (wact << 8) | (Wj << 16);
+            hdr[4 * s + 3] = K8;
+            mbar_arrive(b_hdr + 8 * s);
+            mbar_arrive_expect_tx(b_fa + 8 * s, NSL * A_SLICE);
+            bulk_g2s(smem_u32(smem + s * C::STAGE_BYTES), phiq + (cbase + k0 / KC) * (int64_t)(NSL * A_SLICE),
+                     NSL * A_SLICE, b_fa + 8 * s);
+          }
+          __syncwarp();
+          ++t;
+        }
+      }
+    }
+    for (int e = 0; e < NGRP; ++e) {  // one DONE stage per gather group (the other roles stop at the first)
+      const int s = t % NST;
+      acquire(s);
+      if (lane == 0) {
+        hdr[4 * s + 2] = F_DONE;
+        mbar_arrive(b_hdr + 8 * s);
+      }
+      __syncwarp();
+      ++t;
+    }
+  } else if (warp == W_MMA) {
+    // ------------------------------------------------------------------ MMA issuer
+    uint32_t t = 0, tile = 0;
+    uint64_t da[NST], db[NST];
+#pragma unroll
+    for (int s = 0; s < NST; ++s) {
+      da[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES), 128, 512);
+      db[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE), 128, 512);
+    }
+    for (;;) {
+      const int s = t % NST;
+      const uint32_t ph = (t / NST) & 1;
+      mbar_wait(b_hdr + 8 * s, ph);
+      const int h2 = hdr[4 * s + 2];
+      if (h2 & F_DONE) break;
+      const int wact = (h2 >> 8) & 0xff;
+      if ((h2 & F_FIRST) && tile > 0) mbar_wait(b_tempty, (tile - 1) & 1);  // the epilogue has drained the accumulators
+      mbar_wait(b_fa + 8 * s, ph);
+      mbar_wait(b_fb + 8 * s, ph);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint32_t idesc = umma_idesc_s8_mn(wact);
+        const uint32_t keep = (h2 & F_FIRST) ? 0u : 1u;
+        uint64_t a = da[0], b = db[0];
+#pragma unroll
+        for (int q = 1; q < NST; ++q)
+          if (s == q) { a = da[q]; b = db[q]; }
+#pragma unroll
+        for (int c = 0; c < NSL; ++c)
+#pragma unroll
+          for (int i = 0; i <= c; ++i)
+            umma_i8(tmem + c * NT, a + (uint64_t)(i * (A_SLICE >> 4)), b + (uint64_t)((c - i) * (B_SLICE >> 4)), idesc,
+                    i == 0 ? keep : 1u);
+        umma_commit(b_empty + 8 * s);
+        if (h2 & F_LAST_TILE) umma_commit(b_tfull);
+      }
+      __syncwarp();
+      if (h2 & F_LAST_TILE) ++tile;
+      ++t;
+    }
+  } else if (warp >= W_GATHER0 && warp < W_EPI0) {
+    // ------------------------------------------------------------------ B builders
+    const int grp = (warp - W_GATHER0) / NCH, c = (warp - W_GATHER0) % NCH;
+    int32_t coff[16];  // element offsets of this warp's 16 tile columns in a row of Dq (-1: beyond the panel)
+    int cur_p = -1, cur_n0 = -1;
+    for (uint32_t t = grp;; t += NGRP) {
+      const int s = t % NST;
+      const uint32_t ph = (t / NST) & 1;
+      mbar_wait(b_hdr + 8 * s, ph);
+      const int h2 = hdr[4 * s + 2];
+      if (h2 & F_DONE) break;
+      const int p = hdr[4 * s + 0], h1 = hdr[4 * s + 1], K8 = hdr[4 * s + 3];
+      const int n0 = h1 & 0xffff, k0 = h1 >> 16, wact = (h2 >> 8) & 0xff;
+      if (16 * c < wact) {
+        const int64_t base = panel_off[p];
+        if (p != cur_p || n0 != cur_n0) {
+          cur_p = p;
+          cur_n0 = n0;
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const int n = n0 + 16 * c + j;
+            coff[j] = n < K8 ? colidx[base + n] : -1;
+          }
+        }
+        const int k = k0 + lane;
+        const unsigned long long* row = k < K8 ? Dq + (int64_t)colidx[base + k] * n_ao : nullptr;
+        unsigned long long q[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) q[j] = (row && coff[j] >= 0) ? row[coff[j]] : 0ull;
+        const uint32_t dst = smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE) + c * 512 + lane * 16;
+        // byte transposition: word w of plane i holds digit i of the columns 4w .. 4w+3
+#pragma unroll
+        for (int i0 = 0; i0 < NSL; i0 += 4) {
+          uint32_t o[4][4];
+#pragma unroll
+          for (int w = 0; w < 4; ++w) {
+            uint32_t x0, x1, x2, x3;
+            if (i0 == 0) {
+              x0 = (uint32_t)q[4 * w]; x1 = (uint32_t)q[4 * w + 1]; x2 = (uint32_t)q[4 * w + 2]; x3 = (uint32_t)q[4 * w + 3];
+            } else {
+              x0 = (uint32_t)(q[4 * w] >> 32); x1 = (uint32_t)(q[4 * w + 1] >> 32);
+              x2 = (uint32_t)(q[4 * w + 2] >> 32); x3 = (uint32_t)(q[4 * w + 3] >> 32);
+            }
+            const uint32_t a = __byte_perm(x0, x1, 0x5140), b = __byte_perm(x2, x3, 0x5140);
+            o[0][w] = __byte_perm(a, b, 0x5410);
+            o[1][w] = __byte_perm(a, b, 0x7632);
+            if (i0 + 2 < NSL) {
+              const uint32_t e = __byte_perm(x0, x1, 0x7362), f = __byte_perm(x2, x3, 0x7362);
+              o[2][w] = __byte_perm(e, f, 0x5410);
+              o[3][w] = __byte_perm(e, f, 0x7632);
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            if (i0 + i < NSL)
+              asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + (i0 + i) * B_SLICE), "r"(o[i][0]),
+                           "r"(o[i][1]), "r"(o[i][2]), "r"(o[i][3])
+                           : "memory");
+        }
+        fence_proxy_async_smem();
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_fb + 8 * s);
+    }
+  } else if (warp >= W_EPI0) {
+    // ------------------------------------------------------------------ epilogue
+    const int ew = warp - W_EPI0;  // = warp % 4: TMEM lanes 32 ew .. 32 ew + 31
+    const int g = 32 * ew + lane;
+    double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + ew * NT;
+    const uint32_t tl = tmem + ((uint32_t)(32 * ew) << 16);
+    double rs = 0.0;
+    uint32_t tile = 0;
+    for (uint32_t t = 0;; ++t) {
+      const int s = t % NST;
+      mbar_wait(b_hdr + 8 * s, (t / NST) & 1);
+      const int h2 = hdr[4 * s + 2];
+      if (h2 & F_DONE) break;
+      const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1] & 0xffff, K8 = hdr[4 * s + 3];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_empty + 8 * s);  // header read
+      if (!(h2 & F_LAST_TILE)) continue;
+      const int wj = min((h2 >> 16) & 0xff, K8 - n0);  // real columns of the tile (the store holds K8 per panel)
+      const int64_t base = panel_off[p];
+      for (int j = lane; j < wj; j += 32) tau_s[j] = tau[colidx[base + n0 + j]];
+      __syncwarp();
+      const double* pg = phi + (base + n0) * GB + g;
+      double f[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) f[j] = j < wj ? pg[(int64_t)j * GB] : 0.0;
+      mbar_wait(b_tfull, tile & 1);
+      tc_fence_after();
+      for (int j0 = 0; j0 < wj; j0 += 8) {
+        int32_t acc[NSL][8];
+#pragma unroll
+        for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
+        double fn[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) fn[j] = j0 + 8 + j < wj ? pg[(int64_t)(j0 + 8 + j) * GB] : 0.0;
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          long long x = 0;
+#pragma unroll
+          for (int c = 0; c < NSL; ++c) x = x * 256 + (long long)acc[c][j];
+          const double tj = j0 + j < wj ? tau_s[j0 + j] : 0.0;
+          rs = fma(f[j] * tj, (double)x, rs);
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) f[j] = fn[j];
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_tempty);
+      ++tile;
+      if (h2 & F_LAST_PANEL) {
+        rho_s[(int64_t)p * GB + g] = 2.0 * sigma[(int64_t)p * GB + g] * scalbn(rs, -8 * (NSL + 1));
+        rs = 0.0;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == W_TMEM) tmem_dealloc(tmem, C::TMEM_COLS);
+}
+
+}  // namespace tc
+
+// ------------------------------------------------------------------------------------------------ host side
+template <int NSL>
+static kldi_status tc_prepare(kldi_plan* P) {
+  if (P->d_phiq) return KLDI_OK;
+  if (P->stats.max_k > 16384) {
+    set_error("KLDI_OPT_RHO_TC: a grid block retains %lld AO columns; the int32 accumulators hold 16384", (long long)P->stats.max_k);
+    return KLDI_ESTATE;
+  }
+  std::vector<int64_t> h_chunk(P->n_blocks + 1, 0);
+  for (int64_t p = 0; p < P->n_blocks; ++p) {
+    const int64_t k8 = P->h_panel_off[p + 1] - P->h_panel_off[p];
+    h_chunk[p + 1] = h_chunk[p] + (k8 + tc::KC - 1) / tc::KC;
+  }
+  P->tc_chunks = h_chunk[P->n_blocks];
+  KLDI_CUDA(cudaMalloc(&P->d_chunk_off, sizeof(int64_t) * (P->n_blocks + 1)));
+  KLDI_CUDA(cudaMemcpyAsync(P->d_chunk_off, h_chunk.data(), sizeof(int64_t) * (P->n_blocks + 1), cudaMemcpyHostToDevice, P->stream));
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));  // h_chunk goes out of scope
+  KLDI_CUDA(cudaMalloc(&P->d_sigma, sizeof(double) * P->n_pad));
+  KLDI_CUDA(cudaMalloc(&P->d_phiq, (size_t)std::max<int64_t>(1, P->tc_chunks) * NSL * tc::A_SLICE));
+  KLDI_CUDA(cudaMalloc(&P->d_Dq, sizeof(unsigned long long) * (size_t)P->n_ao * P->n_ao));
+  KLDI_CUDA(cudaMalloc(&P->d_tau, sizeof(double) * 2 * P->n_ao));
+  if (P->n_tasks > 0) {
+    tc::k_slice_phi<NSL><<<P->n_tasks, 128, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_phi,
+                                                           P->d_sigma, P->d_phiq);
+    KLDI_CUDA(cudaGetLastError());
+  }
+  KLDI_CUDA(cudaFuncSetAttribute(tc::k_rho_i8<NSL>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NSL>::SMEM_BYTES));
+  P->stats.phi_bytes += (int64_t)P->tc_chunks * NSL * tc::A_SLICE;
+  return KLDI_OK;
+}
+
+// rho_s of every grid block from D' in P->d_Dp (written by launch_permute_D in its triangular form).
+kldi_status launch_rho_tc(kldi_plan* P) {
+  constexpr int NSL = 5;
+  kldi_status rc = tc_prepare<NSL>(P);
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  const int n = P->n_ao;
+  double* cmax = P->d_tau + n;
+  KLDI_CUDA(cudaMemsetAsync(cmax, 0, sizeof(double) * n, P->stream));
+  tc::k_colmax<<<dim3((n + 31) / 32, (n + 255) / 256), 256, 0, P->stream>>>(P->d_Dp, n, reinterpret_cast<unsigned long long*>(cmax));
+  KLDI_CUDA(cudaGetLastError());
+  tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq);
+  KLDI_CUDA(cudaGetLastError());
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phi, P->d_phiq,
+      P->d_sigma, P->d_Dq, P->d_tau, n, P->d_rho_s);
+  KLDI_CUDA(cudaGetLastError());
+  return KLDI_OK;
+}
+
+}  // namespace kldi
