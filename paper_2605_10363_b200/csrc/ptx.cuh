@@ -69,9 +69,9 @@ __device__ __forceinline__ uint64_t umma_smem_desc(uint32_t saddr, uint32_t lbo,
   return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo >> 4) & 0x3fff) << 16) |
          ((uint64_t)((sbo >> 4) & 0x3fff) << 32) | (1ull << 46);
 }
-// Instruction descriptor of kind::i8: signed 8-bit A and B, both MN-major, 32-bit integer accumulators, M = 128.
-__device__ __forceinline__ uint32_t umma_idesc_s8_mn(int n) {
-  return (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+// Instruction descriptor of kind::i8: signed 8-bit A (K-major) and B (MN-major), 32-bit integer accumulators, M = 128.
+__device__ __forceinline__ uint32_t umma_idesc_s8(int n) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
 }
 // D[tmem] (+)= A[smem] * B[smem], M = 128, K = 32 (int8); issued by ONE thread.  SASS: UTCIMMA.
 __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
@@ -107,6 +107,12 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, int32_t (&r)[8]) {
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // generic-proxy shared-memory writes -> visible to the async proxy (tensor core operand reads)
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// byte b of w, sign-extended to 32 bits: one PRMT with the sign-replicate selector bit (__byte_perm drops it)
+__device__ __forceinline__ int sext_byte(uint32_t w, int b) {  // b folds to an immediate in unrolled code
+  int r;
+  asm("prmt.b32 %0, %1, %1, %2;" : "=r"(r) : "r"(w), "r"(0x8880 + 0x1111 * b));
+  return r;
+}
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile(

@@ -37,19 +37,29 @@ enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
 template <int NSL>
 struct Cfg {
   static constexpr int STAGE_BYTES = NSL * (A_SLICE + B_SLICE);
-  static constexpr int OFF_HDR = NST * STAGE_BYTES;          // [NST][4] int
-  static constexpr int OFF_BAR = OFF_HDR + NST * 16;         // hdr_full[NST], full_a[NST], full_b[NST], empty[NST], tmem_full, tmem_empty
-  static constexpr int OFF_TMEM = OFF_BAR + (4 * NST + 2) * 8;
-  static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;  // [4 epilogue warps][NT] double
+  static constexpr int OFF_EPI = NST * STAGE_BYTES;                   // digit planes of the tile's own columns (epilogue)
+  static constexpr int EPI_BYTES = (NT / KC) * NSL * A_SLICE;
+  static constexpr int OFF_HDR = OFF_EPI + EPI_BYTES;                 // [NST][4] int
+  static constexpr int OFF_KIDX = OFF_HDR + NST * 16;                 // [NST][32] int: plan AO index of the stage's K rows
+  static constexpr int OFF_CIDX = OFF_KIDX + NST * KC * 4;            // [4][NT] int: plan AO index of the tile's columns
+  static constexpr int OFF_BAR = OFF_CIDX + 4 * NT * 4;               // hdr_full, full_a, full_b, empty [NST]; tmem_full, tmem_empty, epi_full, epi_empty
+  static constexpr int OFF_TMEM = OFF_BAR + (4 * NST + 4) * 8;
+  static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;          // [4 epilogue warps][NT] double
   static constexpr int SMEM_BYTES = OFF_TAU + 4 * NT * 8;
   static constexpr int TMEM_COLS = 512;
   static_assert(NSL * NT <= 512, "accumulator classes do not fit tensor memory");
+  static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
-// byte offset of (row m of 128 | column n of the tile, k of the chunk) inside one MN-major digit plane
-__host__ __device__ __forceinline__ int plane_off(int mn, int k) {
-  return (mn >> 4) * 512 + (k >> 3) * 128 + (k & 7) * 16 + (mn & 15);
+// Digit plane of a 128 x 32 Phi chunk, K-major core matrices (8 rows x 16 consecutive K bytes = 128 contiguous bytes):
+// the 16 digits of one grid row and 16 consecutive columns are ONE 16-byte word, which is what the epilogue (one lane =
+// one grid row) reads back.  Descriptor strides: 128 B between the two K halves (lbo), 256 B between 8-row groups (sbo).
+__host__ __device__ __forceinline__ int plane_off_a(int m, int k) {
+  return (m >> 3) * 256 + (k >> 4) * 128 + (m & 7) * 16 + (k & 15);
 }
+// Digit plane of a 32 x 96 D' tile, MN-major core matrices (8 K rows x 16 consecutive N bytes): a gather lane (one K
+// row, 16 columns) writes ONE 16-byte word per plane.  Strides: 128 B between 8-row K groups (lbo), 512 B between
+// 16-column groups (sbo).
 
 // ------------------------------------------------------------------------------------------------ plan side
 // Digit planes of Phi: per grid block the row scales sigma_g, then for every chunk of 32 packed columns NSL planes of
@@ -77,7 +87,7 @@ __global__ void __launch_bounds__(128) k_slice_phi(const int32_t* __restrict__ t
 #pragma unroll
       for (int i = NSL - 1; i >= 0; --i) {  // balanced base-256 digits, least significant first
         const int d = (int)(signed char)(n & 0xff);
-        tile[i * A_SLICE + plane_off(g, kk)] = (unsigned char)d;
+        tile[i * A_SLICE + plane_off_a(g, kk)] = (unsigned char)d;
         n = (n - d) >> 8;
       }
     }
@@ -127,27 +137,35 @@ __global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, 
 // ------------------------------------------------------------------------------------------------ the contraction
 // Persistent, one CTA per SM, warp-specialised:
 //   warp 0      scheduler + A producer: pulls grid blocks from the atomic ticket, walks the block's
-//               (N-tile, K-chunk) stages, writes the stage header and bulk-copies the chunk's NSL digit planes of Phi
+//               (N-tile, K-chunk) stages, writes the stage header and the AO indices of the stage's K rows (and, per
+//               tile, of its columns), bulk-copies the chunk's NSL digit planes of Phi, and after the last stage of a
+//               tile the digit planes of the tile's OWN columns into the epilogue buffer
 //   warps 4-15  B builders, two groups of six on alternate stages: warp c of a group gathers the 16 columns
 //               [n0+16c, n0+16c+16) x 32 rows of D' (lane = K row, 16 x 8-byte digit words), transposes the bytes to
-//               digit planes with PRMT and stores them in the MN-major core-matrix layout (5 x 16-byte stores)
+//               digit planes with PRMT and stores them in the MN-major core-matrix layout (NSL x 16-byte stores)
 //   warp 1      MMA issuer: one elected lane issues the NSL(NSL+1)/2 tcgen05.mma of a stage (A_i x B_j -> class i+j)
 //               and commits them to the stage's empty barrier (and to tmem_full after the last chunk of a tile)
-//   warps 16-19 epilogue: TMEM -> registers (one lane = one grid row), int64 recombination of the classes, FP64
-//               rho += tau_n Phi(g,n) X_int(g,n) with Phi from the FP64 store; rho_p at the end of the panel
+//   warps 16-19 epilogue: TMEM -> registers (one lane = one grid row), int64 recombination of the classes and of the
+//               row's Phi digits (epilogue buffer), FP64 rho += tau_n Phi_int(g,n) X_int(g,n); rho_p at the end of
+//               the panel.  No FP64 Phi is read: the digit planes are the only Phi traffic of the kernel.
+// D' is lower triangular in packed order, so only the chunks k0 >= n0 reach tile [n0, n0+Wj) and chunk [k0, k0+32)
+// only its columns n < k0 + 32; the chunks are walked in DESCENDING k0, so the first one is full width and overwrites
+// (zeroes) every accumulator column of the tile.
 template <int NSL>
 __global__ void __launch_bounds__(NTHREADS, 1)
     k_rho_i8(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket, const int32_t* __restrict__ kp,
              const int64_t* __restrict__ panel_off, const int64_t* __restrict__ chunk_off,
-             const int32_t* __restrict__ colidx, const double* __restrict__ phi, const unsigned char* __restrict__ phiq,
+             const int32_t* __restrict__ colidx, const unsigned char* __restrict__ phiq,
              const double* __restrict__ sigma, const unsigned long long* __restrict__ Dq, const double* __restrict__ tau,
              int n_ao, double* __restrict__ rho_s) {
   using C = Cfg<NSL>;
   extern __shared__ __align__(128) unsigned char smem[];
   volatile int* hdr = reinterpret_cast<volatile int*>(smem + C::OFF_HDR);
+  volatile int* kidx = reinterpret_cast<volatile int*>(smem + C::OFF_KIDX);
+  volatile int* cidx = reinterpret_cast<volatile int*>(smem + C::OFF_CIDX);
   const uint32_t bar0 = smem_u32(smem + C::OFF_BAR);
   const uint32_t b_hdr = bar0, b_fa = bar0 + 8 * NST, b_fb = bar0 + 16 * NST, b_empty = bar0 + 24 * NST;
-  const uint32_t b_tfull = bar0 + 32 * NST, b_tempty = b_tfull + 8;
+  const uint32_t b_tfull = bar0 + 32 * NST, b_tempty = b_tfull + 8, b_efull = b_tfull + 16, b_eempty = b_tfull + 24;
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + C::OFF_TMEM);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) {
@@ -159,6 +177,8 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     }
     mbar_init(b_tfull, 1);
     mbar_init(b_tempty, 4);
+    mbar_init(b_efull, 1);
+    mbar_init(b_eempty, 4);
     fence_mbar_init();
   }
   if (warp == W_TMEM) tmem_alloc(smem_u32(smem + C::OFF_TMEM), C::TMEM_COLS);
@@ -169,10 +189,8 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 
   if (warp == W_PROD) {
     // ------------------------------------------------------------------ scheduler + A producer
-    uint32_t t = 0;  // stage sequence number: slot t % NST, use t / NST
-    auto acquire = [&](int s) {
-      if (t >= NST) mbar_wait(b_empty + 8 * s, ((t / NST) - 1) & 1);
-    };
+    uint32_t t = 0;     // stage sequence number: slot t % NST, use t / NST
+    uint32_t tile = 0;  // tile sequence number
     for (;;) {
       int task = 0;
       if (lane == 0) task = atomicAdd(ticket, 1);
@@ -180,25 +198,36 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       if (task >= n_tasks) break;
       const int p = tasks[task];
       const int K8 = (kp[p] + 7) & ~7, K32 = (K8 + KC - 1) & ~(KC - 1);
-      const int64_t cbase = chunk_off[p];
+      const int64_t base = panel_off[p], cbase = chunk_off[p];
       const int ntile = (K32 + NT - 1) / NT;
       const int W = ((K32 / KC + ntile - 1) / ntile) * KC;  // tiles start on chunk boundaries
-      for (int jt = 0; jt < ntile; ++jt) {
+      for (int jt = 0; jt < ntile; ++jt, ++tile) {
         const int n0 = jt * W, Wj = min(W, K32 - n0);
-        // D' is lower triangular in packed order: only the chunks k0 >= n0 reach this tile, and chunk [k0, k0+32)
-        // only its columns n < k0 + 32
-        for (int k0 = n0; k0 < K32; k0 += KC) {
+        int cn[NT / 32];
+#pragma unroll
+        for (int u = 0; u < NT / 32; ++u) {
+          const int n = n0 + lane + 32 * u;
+          cn[u] = (lane + 32 * u < Wj && n < K8) ? colidx[base + n] : -1;
+        }
+        for (int k0 = K32 - KC; k0 >= n0; k0 -= KC) {
           const int s = t % NST;
-          acquire(s);
+          const int k = k0 + lane;
+          const int kr = k < K8 ? colidx[base + k] : -1;
+          if (t >= NST) mbar_wait(b_empty + 8 * s, ((t / NST) - 1) & 1);
+          kidx[s * KC + lane] = kr;
+          if (k0 == K32 - KC) {  // a tile's column indices live 4 tiles: every tile has at least one stage
+#pragma unroll
+            for (int u = 0; u < NT / 32; ++u) cidx[(tile & 3) * NT + lane + 32 * u] = cn[u];
+          }
+          __syncwarp();
           if (lane == 0) {
             int fl = 0;
-            if (k0 == n0) fl |= F_FIRST;
-            if (k0 + KC >= K32) fl |= F_LAST_TILE | (jt == ntile - 1 ? F_LAST_PANEL : 0);
-            // the first chunk of a tile runs at full width: it overwrites (zeroes) every accumulator column of the tile
-            const int wact = k0 == n0 ? Wj : min(Wj, k0 + KC - n0);
+            if (k0 == K32 - KC) fl |= F_FIRST;
+            if (k0 == n0) fl |= F_LAST_TILE | (jt == ntile - 1 ? F_LAST_PANEL : 0);
+            const int wact = min(Wj, k0 + KC - n0);
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = n0 | (k0 << 16);
-            hdr[4 * s + 2] = fl | (wact << 8) | (Wj << 16);
+            hdr[4 * s + 2] = fl | (wact << 8) | (Wj << 16) | ((tile & 3) << 24);
             hdr[4 * s + 3] = K8;
             mbar_arrive(b_hdr + 8 * s);
             mbar_arrive_expect_tx(b_fa + 8 * s, NSL * A_SLICE);
@@ -208,11 +237,19 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           __syncwarp();
           ++t;
         }
+        // the digit planes of the tile's own columns for its epilogue (single buffer: wait for the previous epilogue)
+        if (tile > 0) mbar_wait(b_eempty, (tile - 1) & 1);
+        if (lane == 0) {
+          const uint32_t bytes = (uint32_t)(Wj / KC) * (NSL * A_SLICE);
+          mbar_arrive_expect_tx(b_efull, bytes);
+          bulk_g2s(smem_u32(smem + C::OFF_EPI), phiq + (cbase + n0 / KC) * (int64_t)(NSL * A_SLICE), bytes, b_efull);
+        }
+        __syncwarp();
       }
     }
     for (int e = 0; e < NGRP; ++e) {  // one DONE stage per gather group (the other roles stop at the first)
       const int s = t % NST;
-      acquire(s);
+      if (t >= NST) mbar_wait(b_empty + 8 * s, ((t / NST) - 1) & 1);
       if (lane == 0) {
         hdr[4 * s + 2] = F_DONE;
         mbar_arrive(b_hdr + 8 * s);
@@ -226,7 +263,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     uint64_t da[NST], db[NST];
 #pragma unroll
     for (int s = 0; s < NST; ++s) {
-      da[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES), 128, 512);
+      da[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES), 128, 256);
       db[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE), 128, 512);
     }
     for (;;) {
@@ -241,7 +278,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       mbar_wait(b_fb + 8 * s, ph);
       tc_fence_after();
       if (elect_one()) {
-        const uint32_t idesc = umma_idesc_s8_mn(wact);
+        const uint32_t idesc = umma_idesc_s8(wact);
         const uint32_t keep = (h2 & F_FIRST) ? 0u : 1u;
         uint64_t a = da[0], b = db[0];
 #pragma unroll
@@ -263,32 +300,23 @@ __global__ void __launch_bounds__(NTHREADS, 1)
   } else if (warp >= W_GATHER0 && warp < W_EPI0) {
     // ------------------------------------------------------------------ B builders
     const int grp = (warp - W_GATHER0) / NCH, c = (warp - W_GATHER0) % NCH;
-    int32_t coff[16];  // element offsets of this warp's 16 tile columns in a row of Dq (-1: beyond the panel)
-    int cur_p = -1, cur_n0 = -1;
     for (uint32_t t = grp;; t += NGRP) {
       const int s = t % NST;
       const uint32_t ph = (t / NST) & 1;
       mbar_wait(b_hdr + 8 * s, ph);
       const int h2 = hdr[4 * s + 2];
       if (h2 & F_DONE) break;
-      const int p = hdr[4 * s + 0], h1 = hdr[4 * s + 1], K8 = hdr[4 * s + 3];
-      const int n0 = h1 & 0xffff, k0 = h1 >> 16, wact = (h2 >> 8) & 0xff;
+      const int wact = (h2 >> 8) & 0xff;
       if (16 * c < wact) {
-        const int64_t base = panel_off[p];
-        if (p != cur_p || n0 != cur_n0) {
-          cur_p = p;
-          cur_n0 = n0;
-#pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const int n = n0 + 16 * c + j;
-            coff[j] = n < K8 ? colidx[base + n] : -1;
-          }
-        }
-        const int k = k0 + lane;
-        const unsigned long long* row = k < K8 ? Dq + (int64_t)colidx[base + k] * n_ao : nullptr;
+        const int kr = kidx[s * KC + lane];
+        const volatile int* cn = cidx + ((h2 >> 24) & 3) * NT + 16 * c;
+        const unsigned long long* row = Dq + (int64_t)max(kr, 0) * n_ao;
         unsigned long long q[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) q[j] = (row && coff[j] >= 0) ? row[coff[j]] : 0ull;
+        for (int j = 0; j < 16; ++j) {
+          const int cj = cn[j];
+          q[j] = (kr >= 0 && cj >= 0) ? __ldg(row + cj) : 0ull;
+        }
         const uint32_t dst = smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE) + c * 512 + lane * 16;
         // byte transposition: word w of plane i holds digit i of the columns 4w .. 4w+3
 #pragma unroll
@@ -330,6 +358,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     const int g = 32 * ew + lane;
     double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + ew * NT;
     const uint32_t tl = tmem + ((uint32_t)(32 * ew) << 16);
+    const unsigned char* eg = smem + C::OFF_EPI + (g >> 3) * 256 + (g & 7) * 16;  // this row's 16-byte words
     double rs = 0.0;
     uint32_t tile = 0;
     for (uint32_t t = 0;; ++t) {
@@ -341,41 +370,50 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       __syncwarp();
       if (lane == 0) mbar_arrive(b_empty + 8 * s);  // header read
       if (!(h2 & F_LAST_TILE)) continue;
-      const int wj = min((h2 >> 16) & 0xff, K8 - n0);  // real columns of the tile (the store holds K8 per panel)
-      const int64_t base = panel_off[p];
-      for (int j = lane; j < wj; j += 32) tau_s[j] = tau[colidx[base + n0 + j]];
+      const int wj = min((h2 >> 16) & 0xff, K8 - n0);  // real columns of the tile
+      const volatile int* cn = cidx + ((h2 >> 24) & 3) * NT;
+      for (int j = lane; j < wj; j += 32) tau_s[j] = tau[cn[j]];
       __syncwarp();
-      const double* pg = phi + (base + n0) * GB + g;
-      double f[8];
-#pragma unroll
-      for (int j = 0; j < 8; ++j) f[j] = j < wj ? pg[(int64_t)j * GB] : 0.0;
+      mbar_wait(b_efull, tile & 1);
       mbar_wait(b_tfull, tile & 1);
       tc_fence_after();
-      for (int j0 = 0; j0 < wj; j0 += 8) {
-        int32_t acc[NSL][8];
+      for (int j0 = 0; j0 < wj; j0 += 16) {
+        uint4 dg[NSL];  // digit i of this row for the columns j0 .. j0+15
 #pragma unroll
-        for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
-        double fn[8];
+        for (int i = 0; i < NSL; ++i)
+          dg[i] = *reinterpret_cast<const uint4*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) fn[j] = j0 + 8 + j < wj ? pg[(int64_t)(j0 + 8 + j) * GB] : 0.0;
-        tmem_ld_wait();
+        for (int h = 0; h < 2; ++h) {
+          if (j0 + 8 * h < wj) {
+            int32_t acc[NSL][8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          long long x = 0;
+            for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0 + 8 * h, acc[c]);
+            tmem_ld_wait();
 #pragma unroll
-          for (int c = 0; c < NSL; ++c) x = x * 256 + (long long)acc[c][j];
-          const double tj = j0 + j < wj ? tau_s[j0 + j] : 0.0;
-          rs = fma(f[j] * tj, (double)x, rs);
+            for (int j = 0; j < 8; ++j) {
+              long long x = 0, f = 0;
+#pragma unroll
+              for (int c = 0; c < NSL; ++c) {
+                x = x * 256 + (long long)acc[c][j];
+                const uint32_t w = (2 * h + (j >> 2)) == 0 ? dg[c].x : (2 * h + (j >> 2)) == 1 ? dg[c].y
+                                   : (2 * h + (j >> 2)) == 2 ? dg[c].z : dg[c].w;
+                f = f * 256 + (long long)sext_byte(w, j & 3);
+              }
+              rs = fma((double)f * tau_s[j0 + 8 * h + j], (double)x, rs);
+            }
+          }
         }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) f[j] = fn[j];
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(b_tempty);
+      if (lane == 0) {
+        mbar_arrive(b_tempty);
+        mbar_arrive(b_eempty);
+      }
       ++tile;
       if (h2 & F_LAST_PANEL) {
-        rho_s[(int64_t)p * GB + g] = 2.0 * sigma[(int64_t)p * GB + g] * scalbn(rs, -8 * (NSL + 1));
+        const double sg = sigma[(int64_t)p * GB + g];
+        rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs, -8 * (2 * NSL + 1));
         rs = 0.0;
       }
     }
@@ -435,8 +473,8 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   KLDI_CUDA(cudaGetLastError());
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
-      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phi, P->d_phiq,
-      P->d_sigma, P->d_Dq, P->d_tau, n, P->d_rho_s);
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phiq, P->d_sigma,
+      P->d_Dq, P->d_tau, n, P->d_rho_s);
   KLDI_CUDA(cudaGetLastError());
   return KLDI_OK;
 }
