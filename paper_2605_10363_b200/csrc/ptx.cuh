@@ -69,9 +69,9 @@ __device__ __forceinline__ uint64_t umma_smem_desc(uint32_t saddr, uint32_t lbo,
   return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo >> 4) & 0x3fff) << 16) |
          ((uint64_t)((sbo >> 4) & 0x3fff) << 32) | (1ull << 46);
 }
-// Instruction descriptor of kind::i8: signed 8-bit A (K-major) and B (MN-major), 32-bit integer accumulators, M = 128.
+// Instruction descriptor of kind::i8: signed 8-bit A and B, both K-major, 32-bit integer accumulators, M = 128.
 __device__ __forceinline__ uint32_t umma_idesc_s8(int n) {
-  return (2u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+  return (2u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (0u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
 }
 // D[tmem] (+)= A[smem] * B[smem], M = 128, K = 32 (int8); issued by ONE thread.  SASS: UTCIMMA.
 __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,

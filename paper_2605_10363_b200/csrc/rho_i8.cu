@@ -25,13 +25,14 @@ namespace tc {
 constexpr int KC = 32;                       // K per tcgen05.mma kind::i8 = packed columns per ring stage
 constexpr int NT = 96;                       // N-tile width (NSL * NT <= 512 TMEM columns for NSL = 5)
 constexpr int A_SLICE = GB * KC;             // 4096 B: one digit plane of a 128 x 32 Phi chunk
-constexpr int NCH = NT / 16;                 // 16-column pieces of the B tile = gather warps per group
-constexpr int B_SLICE = NCH * 512;           // 3072 B: one digit plane of a 32 x 96 D' tile
+constexpr int NCH = 2 * (NT / 32);           // gather units of a stage (32 columns x 16 K rows) = gather warps per group
+constexpr int B_SLICE = (NT / 8) * 256;      // 3072 B: one digit plane of a 32 x 96 D' tile
 constexpr int NST = 4;                       // ring stages
 constexpr int NGRP = 2;                      // gather groups (alternate stages)
-constexpr int W_PROD = 0, W_MMA = 1, W_TMEM = 2, W_GATHER0 = 4, W_EPI0 = W_GATHER0 + NGRP * NCH;  // warp roles
-constexpr int NWARPS = W_EPI0 + 4;
-constexpr int NTHREADS = 32 * NWARPS;        // 640
+constexpr int NEPI = 8;                      // epilogue warps: two per TMEM lane quarter, alternate 8-column groups
+constexpr int W_PROD = 0, W_MMA = 1, W_GATHER0 = 2, W_EPI0 = W_GATHER0 + NGRP * NCH;  // warp roles
+constexpr int NWARPS = W_EPI0 + NEPI;
+constexpr int NTHREADS = 32 * NWARPS;        // 704
 enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
 
 template <int NSL>
@@ -44,8 +45,9 @@ struct Cfg {
   static constexpr int OFF_CIDX = OFF_KIDX + NST * KC * 4;            // [4][NT] int: plan AO index of the tile's columns
   static constexpr int OFF_BAR = OFF_CIDX + 4 * NT * 4;               // hdr_full, full_a, full_b, empty [NST]; tmem_full, tmem_empty, epi_full, epi_empty
   static constexpr int OFF_TMEM = OFF_BAR + (4 * NST + 4) * 8;
-  static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;          // [4 epilogue warps][NT] double
-  static constexpr int SMEM_BYTES = OFF_TAU + 4 * NT * 8;
+  static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;          // [NEPI epilogue warps][NT] double
+  static constexpr int OFF_RED = OFF_TAU + NEPI * NT * 8;             // [128] double: partial row sums of the second warp set
+  static constexpr int SMEM_BYTES = OFF_RED + GB * 8;
   static constexpr int TMEM_COLS = 512;
   static_assert(NSL * NT <= 512, "accumulator classes do not fit tensor memory");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
@@ -57,9 +59,8 @@ struct Cfg {
 __host__ __device__ __forceinline__ int plane_off_a(int m, int k) {
   return (m >> 3) * 256 + (k >> 4) * 128 + (m & 7) * 16 + (k & 15);
 }
-// Digit plane of a 32 x 96 D' tile, MN-major core matrices (8 K rows x 16 consecutive N bytes): a gather lane (one K
-// row, 16 columns) writes ONE 16-byte word per plane.  Strides: 128 B between 8-row K groups (lbo), 512 B between
-// 16-column groups (sbo).
+// Digit plane of a 32 x 96 D' tile: the same K-major core matrices with the tile column n as the row: a gather lane
+// (one column, 16 consecutive K rows) writes ONE 16-byte word per plane.
 
 // ------------------------------------------------------------------------------------------------ plan side
 // Digit planes of Phi: per grid block the row scales sigma_g, then for every chunk of 32 packed columns NSL planes of
@@ -173,15 +174,15 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       mbar_init(b_hdr + 8 * s, 1);
       mbar_init(b_fa + 8 * s, 1);
       mbar_init(b_fb + 8 * s, NCH);
-      mbar_init(b_empty + 8 * s, 1 + 4);  // tcgen05.commit of the stage's MMAs + the 4 epilogue warps (header read)
+      mbar_init(b_empty + 8 * s, 1 + NEPI);  // tcgen05.commit of the stage's MMAs + the epilogue warps (header read)
     }
     mbar_init(b_tfull, 1);
-    mbar_init(b_tempty, 4);
+    mbar_init(b_tempty, NEPI);
     mbar_init(b_efull, 1);
-    mbar_init(b_eempty, 4);
+    mbar_init(b_eempty, NEPI);
     fence_mbar_init();
   }
-  if (warp == W_TMEM) tmem_alloc(smem_u32(smem + C::OFF_TMEM), C::TMEM_COLS);
+  if (warp == W_MMA) tmem_alloc(smem_u32(smem + C::OFF_TMEM), C::TMEM_COLS);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -264,7 +265,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 #pragma unroll
     for (int s = 0; s < NST; ++s) {
       da[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES), 128, 256);
-      db[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE), 128, 512);
+      db[s] = umma_smem_desc(smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE), 128, 256);
     }
     for (;;) {
       const int s = t % NST;
@@ -297,9 +298,12 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       if (h2 & F_LAST_TILE) ++tile;
       ++t;
     }
-  } else if (warp >= W_GATHER0 && warp < W_EPI0) {
+  } else if (warp < W_EPI0) {
     // ------------------------------------------------------------------ B builders
+    // unit of a warp: 32 tile columns (lane = column) x 16 K rows; an instruction reads ONE row of Dq at the 32
+    // ascending AO indices of consecutive packed columns, so a warp load touches a few 128-byte lines, not 32
     const int grp = (warp - W_GATHER0) / NCH, c = (warp - W_GATHER0) % NCH;
+    const int ng = c >> 1, h = c & 1;
     for (uint32_t t = grp;; t += NGRP) {
       const int s = t % NST;
       const uint32_t ph = (t / NST) & 1;
@@ -307,18 +311,18 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       const int h2 = hdr[4 * s + 2];
       if (h2 & F_DONE) break;
       const int wact = (h2 >> 8) & 0xff;
-      if (16 * c < wact) {
-        const int kr = kidx[s * KC + lane];
-        const volatile int* cn = cidx + ((h2 >> 24) & 3) * NT + 16 * c;
-        const unsigned long long* row = Dq + (int64_t)max(kr, 0) * n_ao;
+      if (32 * ng < wact) {
+        const int cj = cidx[((h2 >> 24) & 3) * NT + 32 * ng + lane];
+        const unsigned long long* col = Dq + max(cj, 0);
         unsigned long long q[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int cj = cn[j];
-          q[j] = (kr >= 0 && cj >= 0) ? __ldg(row + cj) : 0ull;
+        for (int r = 0; r < 16; ++r) {
+          const int kr = kidx[s * KC + 16 * h + r];
+          q[r] = (kr >= 0 && cj >= 0) ? __ldg(col + (int64_t)kr * n_ao) : 0ull;
         }
-        const uint32_t dst = smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE) + c * 512 + lane * 16;
-        // byte transposition: word w of plane i holds digit i of the columns 4w .. 4w+3
+        const uint32_t dst = smem_u32(smem + s * C::STAGE_BYTES + NSL * A_SLICE) + (4 * ng + (lane >> 3)) * 256 + h * 128 +
+                             (lane & 7) * 16;
+        // byte transposition: word w of plane i holds digit i of the K rows 4w .. 4w+3
 #pragma unroll
         for (int i0 = 0; i0 < NSL; i0 += 4) {
           uint32_t o[4][4];
@@ -352,12 +356,14 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       __syncwarp();
       if (lane == 0) mbar_arrive(b_fb + 8 * s);
     }
-  } else if (warp >= W_EPI0) {
+  } else {
     // ------------------------------------------------------------------ epilogue
-    const int ew = warp - W_EPI0;  // = warp % 4: TMEM lanes 32 ew .. 32 ew + 31
-    const int g = 32 * ew + lane;
-    double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + ew * NT;
-    const uint32_t tl = tmem + ((uint32_t)(32 * ew) << 16);
+    const int qd = warp & 3;                 // TMEM lane quarter of this warp
+    const int hs = (warp - W_EPI0) >> 2;     // warp set: 8-column groups with (group & 1) == hs
+    const int g = 32 * qd + lane;
+    double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + (warp - W_EPI0) * NT;
+    double* red = reinterpret_cast<double*>(smem + C::OFF_RED);
+    const uint32_t tl = tmem + ((uint32_t)(32 * qd) << 16);
     const unsigned char* eg = smem + C::OFF_EPI + (g >> 3) * 256 + (g & 7) * 16;  // this row's 16-byte words
     double rs = 0.0;
     uint32_t tile = 0;
@@ -377,31 +383,40 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       mbar_wait(b_efull, tile & 1);
       mbar_wait(b_tfull, tile & 1);
       tc_fence_after();
-      for (int j0 = 0; j0 < wj; j0 += 16) {
-        uint4 dg[NSL];  // digit i of this row for the columns j0 .. j0+15
+      for (int j0 = 8 * hs; j0 < wj; j0 += 16) {
+        uint2 dg[NSL];  // digit i of this row for the columns j0 .. j0+7
 #pragma unroll
         for (int i = 0; i < NSL; ++i)
-          dg[i] = *reinterpret_cast<const uint4*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128);
+          dg[i] = *reinterpret_cast<const uint2*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128 +
+                                                  (j0 & 8));
+        int32_t acc[NSL][8];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          if (j0 + 8 * h < wj) {
-            int32_t acc[NSL][8];
+        for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
+        tmem_ld_wait();
 #pragma unroll
-            for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0 + 8 * h, acc[c]);
-            tmem_ld_wait();
+        for (int j = 0; j < 8; ++j) {
+          int d[NSL];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              long long x = 0, f = 0;
+          for (int c = 0; c < NSL; ++c) d[c] = sext_byte(j < 4 ? dg[c].x : dg[c].y, j & 3);
+          // Phi_int = sum_c d_c 256^(NSL-1-c) and X_int = sum_c acc_c 256^(NSL-1-c), each as high part * 2^24 + low part
+          double fd, xd;
+          if (NSL == 5) {
+            const int fh = d[0] * 256 + d[1], fl = (d[2] * 256 + d[3]) * 256 + d[4];
+            fd = fma((double)fh, 16777216.0, (double)fl);
+            const long long xh = (long long)acc[0][j] * 256 + acc[1][j];
+            const long long xl = ((long long)acc[2][j] * 256 + acc[3][j]) * 256 + acc[4][j];
+            xd = fma((double)xh, 16777216.0, (double)xl);
+          } else {
+            long long f = 0, x = 0;
 #pragma unroll
-              for (int c = 0; c < NSL; ++c) {
-                x = x * 256 + (long long)acc[c][j];
-                const uint32_t w = (2 * h + (j >> 2)) == 0 ? dg[c].x : (2 * h + (j >> 2)) == 1 ? dg[c].y
-                                   : (2 * h + (j >> 2)) == 2 ? dg[c].z : dg[c].w;
-                f = f * 256 + (long long)sext_byte(w, j & 3);
-              }
-              rs = fma((double)f * tau_s[j0 + 8 * h + j], (double)x, rs);
+            for (int c = 0; c < NSL; ++c) {
+              f = f * 256 + d[c];
+              x = x * 256 + acc[c][j];
             }
+            fd = (double)f;
+            xd = (double)x;
           }
+          rs = fma(fd * tau_s[j0 + j], xd, rs);
         }
       }
       tc_fence_before();
@@ -411,16 +426,21 @@ __global__ void __launch_bounds__(NTHREADS, 1)
         mbar_arrive(b_eempty);
       }
       ++tile;
-      if (h2 & F_LAST_PANEL) {
-        const double sg = sigma[(int64_t)p * GB + g];
-        rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs, -8 * (2 * NSL + 1));
+      if (h2 & F_LAST_PANEL) {  // the two warp sets of a row: second set through shared memory, fixed order
+        if (hs == 1) red[g] = rs;
+        asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
+        if (hs == 0) {
+          const double sg = sigma[(int64_t)p * GB + g];
+          rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs + red[g], -8 * (2 * NSL + 1));
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
         rs = 0.0;
       }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == W_TMEM) tmem_dealloc(tmem, C::TMEM_COLS);
+  if (warp == W_MMA) tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
 }  // namespace tc
