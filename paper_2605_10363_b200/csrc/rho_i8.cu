@@ -15,6 +15,7 @@
 // and the epilogue forms rho in FP64 from the int64 recombination and the FP64 Phi store.  NSL = 5: 15 int8 products,
 // max|d rho| ~ 1e-10 on the 8-water case (tolerance 1e-9); NSL = 6: 21 products, ~3e-13.
 #include <cstdio>
+#include <cstdlib>
 
 #include "kldi_internal.h"
 #include "ptx.cuh"
@@ -29,7 +30,11 @@ constexpr int NCH = 2 * (NT / 32);           // gather units of a stage (32 colu
 constexpr int B_SLICE = (NT / 8) * 256;      // 3072 B: one digit plane of a 32 x 96 D' tile
 constexpr int NST = 4;                       // ring stages
 constexpr int NGRP = 2;                      // gather groups (alternate stages)
-constexpr int NEPI = 8;                      // epilogue warps: two per TMEM lane quarter, alternate 8-column groups
+#ifndef KLDI_TC_NEPI
+#define KLDI_TC_NEPI 16
+#endif
+constexpr int NEPI = KLDI_TC_NEPI;           // epilogue warps: NEPI/4 per TMEM lane quarter, 4-column groups dealt round-robin
+constexpr int NSET = NEPI / 4;
 constexpr int W_PROD = 0, W_MMA = 1, W_GATHER0 = 2, W_EPI0 = W_GATHER0 + NGRP * NCH;  // warp roles
 constexpr int NWARPS = W_EPI0 + NEPI;
 constexpr int NTHREADS = 32 * NWARPS;        // 704
@@ -46,8 +51,8 @@ struct Cfg {
   static constexpr int OFF_BAR = OFF_CIDX + 4 * NT * 4;               // hdr_full, full_a, full_b, empty [NST]; tmem_full, tmem_empty, epi_full, epi_empty
   static constexpr int OFF_TMEM = OFF_BAR + (4 * NST + 4) * 8;
   static constexpr int OFF_TAU = (OFF_TMEM + 16 + 15) & ~15;          // [NEPI epilogue warps][NT] double
-  static constexpr int OFF_RED = OFF_TAU + NEPI * NT * 8;             // [128] double: partial row sums of the second warp set
-  static constexpr int SMEM_BYTES = OFF_RED + GB * 8;
+  static constexpr int OFF_RED = OFF_TAU + NEPI * NT * 8;             // [NSET-1][128] double: partial row sums of the other warp sets
+  static constexpr int SMEM_BYTES = OFF_RED + (NSET - 1) * GB * 8;
   static constexpr int TMEM_COLS = 512;
   static_assert(NSL * NT <= 512, "accumulator classes do not fit tensor memory");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
@@ -158,9 +163,20 @@ __global__ void __launch_bounds__(NTHREADS, 1)
              const int64_t* __restrict__ panel_off, const int64_t* __restrict__ chunk_off,
              const int32_t* __restrict__ colidx, const unsigned char* __restrict__ phiq,
              const double* __restrict__ sigma, const unsigned long long* __restrict__ Dq, const double* __restrict__ tau,
-             int n_ao, double* __restrict__ rho_s) {
+             int n_ao, double* __restrict__ rho_s, long long* __restrict__ dbg) {
   using C = Cfg<NSL>;
   extern __shared__ __align__(128) unsigned char smem[];
+  long long tw[6] = {0, 0, 0, 0, 0, 0};  // debug: cycles spent in the waits of this warp's role
+  auto twait = [&](int slot, uint32_t bar, uint32_t parity) {
+    if (dbg) {
+      const long long t0 = clock64();
+      mbar_wait(bar, parity);
+      tw[slot] += clock64() - t0;
+    } else {
+      mbar_wait(bar, parity);
+    }
+  };
+  const long long t_begin = dbg ? clock64() : 0;
   volatile int* hdr = reinterpret_cast<volatile int*>(smem + C::OFF_HDR);
   volatile int* kidx = reinterpret_cast<volatile int*>(smem + C::OFF_KIDX);
   volatile int* cidx = reinterpret_cast<volatile int*>(smem + C::OFF_CIDX);
@@ -214,7 +230,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           const int s = t % NST;
           const int k = k0 + lane;
           const int kr = k < K8 ? colidx[base + k] : -1;
-          if (t >= NST) mbar_wait(b_empty + 8 * s, ((t / NST) - 1) & 1);
+          if (t >= NST) twait(0, b_empty + 8 * s, ((t / NST) - 1) & 1);
           kidx[s * KC + lane] = kr;
           if (k0 == K32 - KC) {  // a tile's column indices live 4 tiles: every tile has at least one stage
 #pragma unroll
@@ -239,7 +255,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           ++t;
         }
         // the digit planes of the tile's own columns for its epilogue (single buffer: wait for the previous epilogue)
-        if (tile > 0) mbar_wait(b_eempty, (tile - 1) & 1);
+        if (tile > 0) twait(1, b_eempty, (tile - 1) & 1);
         if (lane == 0) {
           const uint32_t bytes = (uint32_t)(Wj / KC) * (NSL * A_SLICE);
           mbar_arrive_expect_tx(b_efull, bytes);
@@ -270,13 +286,13 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     for (;;) {
       const int s = t % NST;
       const uint32_t ph = (t / NST) & 1;
-      mbar_wait(b_hdr + 8 * s, ph);
+      twait(0, b_hdr + 8 * s, ph);
       const int h2 = hdr[4 * s + 2];
       if (h2 & F_DONE) break;
       const int wact = (h2 >> 8) & 0xff;
-      if ((h2 & F_FIRST) && tile > 0) mbar_wait(b_tempty, (tile - 1) & 1);  // the epilogue has drained the accumulators
-      mbar_wait(b_fa + 8 * s, ph);
-      mbar_wait(b_fb + 8 * s, ph);
+      if ((h2 & F_FIRST) && tile > 0) twait(1, b_tempty, (tile - 1) & 1);  // the epilogue has drained the accumulators
+      twait(2, b_fa + 8 * s, ph);
+      twait(3, b_fb + 8 * s, ph);
       tc_fence_after();
       if (elect_one()) {
         const uint32_t idesc = umma_idesc_s8(wact);
@@ -307,7 +323,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     for (uint32_t t = grp;; t += NGRP) {
       const int s = t % NST;
       const uint32_t ph = (t / NST) & 1;
-      mbar_wait(b_hdr + 8 * s, ph);
+      twait(0, b_hdr + 8 * s, ph);
       const int h2 = hdr[4 * s + 2];
       if (h2 & F_DONE) break;
       const int wact = (h2 >> 8) & 0xff;
@@ -359,7 +375,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
   } else {
     // ------------------------------------------------------------------ epilogue
     const int qd = warp & 3;                 // TMEM lane quarter of this warp
-    const int hs = (warp - W_EPI0) >> 2;     // warp set: 8-column groups with (group & 1) == hs
+    const int hs = (warp - W_EPI0) >> 2;     // warp set: 4-column groups with group % NSET == hs
     const int g = 32 * qd + lane;
     double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + (warp - W_EPI0) * NT;
     double* red = reinterpret_cast<double*>(smem + C::OFF_RED);
@@ -369,7 +385,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
     uint32_t tile = 0;
     for (uint32_t t = 0;; ++t) {
       const int s = t % NST;
-      mbar_wait(b_hdr + 8 * s, (t / NST) & 1);
+      twait(0, b_hdr + 8 * s, (t / NST) & 1);
       const int h2 = hdr[4 * s + 2];
       if (h2 & F_DONE) break;
       const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1] & 0xffff, K8 = hdr[4 * s + 3];
@@ -380,32 +396,38 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       const volatile int* cn = cidx + ((h2 >> 24) & 3) * NT;
       for (int j = lane; j < wj; j += 32) tau_s[j] = tau[cn[j]];
       __syncwarp();
-      mbar_wait(b_efull, tile & 1);
-      mbar_wait(b_tfull, tile & 1);
+      twait(1, b_efull, tile & 1);
+      twait(2, b_tfull, tile & 1);
       tc_fence_after();
-      for (int j0 = 8 * hs; j0 < wj; j0 += 16) {
-        uint2 dg[NSL];  // digit i of this row for the columns j0 .. j0+7
+      const long long t_e0 = dbg ? clock64() : 0;
+      double rs2 = 0.0;
+      for (int j0 = 4 * hs; j0 < wj; j0 += 4 * NSET) {
+        uint32_t dg[NSL];  // digit i of this row for the columns j0 .. j0+3
 #pragma unroll
         for (int i = 0; i < NSL; ++i)
-          dg[i] = *reinterpret_cast<const uint2*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128 +
-                                                  (j0 & 8));
-        int32_t acc[NSL][8];
+          dg[i] = *reinterpret_cast<const uint32_t*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128 +
+                                                     (j0 & 12));
+        int32_t acc[NSL][4];
 #pragma unroll
-        for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
+        for (int c = 0; c < NSL; ++c) tmem_ld4(tl + c * NT + j0, acc[c]);
+        const double2 t01 = *reinterpret_cast<const double2*>(tau_s + j0), t23 = *reinterpret_cast<const double2*>(tau_s + j0 + 2);
         tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < 4; ++j) {
           int d[NSL];
 #pragma unroll
-          for (int c = 0; c < NSL; ++c) d[c] = sext_byte(j < 4 ? dg[c].x : dg[c].y, j & 3);
-          // Phi_int = sum_c d_c 256^(NSL-1-c) and X_int = sum_c acc_c 256^(NSL-1-c), each as high part * 2^24 + low part
+          for (int c = 0; c < NSL; ++c) d[c] = sext_byte(dg[c], j);
+          // Phi_int = sum_c d_c 256^(NSL-1-c), X_int = sum_c acc_c 256^(NSL-1-c): integer parts below 2^51 go to FP64
+          // through the 2^52 + 2^51 mantissa trick (one integer multiply-add chain + one DADD each)
+          constexpr long long MAGIC = 0x4338000000000000LL;
+          constexpr double MAGIC_D = 6755399441055744.0;
           double fd, xd;
           if (NSL == 5) {
             const int fh = d[0] * 256 + d[1], fl = (d[2] * 256 + d[3]) * 256 + d[4];
-            fd = fma((double)fh, 16777216.0, (double)fl);
-            const long long xh = (long long)acc[0][j] * 256 + acc[1][j];
-            const long long xl = ((long long)acc[2][j] * 256 + acc[3][j]) * 256 + acc[4][j];
-            xd = fma((double)xh, 16777216.0, (double)xl);
+            fd = __longlong_as_double((long long)fh * 16777216 + ((long long)fl + MAGIC)) - MAGIC_D;
+            const long long xh = (long long)acc[0][j] * 65536 + ((long long)acc[1][j] * 256 + ((long long)acc[2][j] + MAGIC));
+            const long long xl = (long long)acc[3][j] * 256 + ((long long)acc[4][j] + MAGIC);
+            xd = fma(__longlong_as_double(xh) - MAGIC_D, 65536.0, __longlong_as_double(xl) - MAGIC_D);
           } else {
             long long f = 0, x = 0;
 #pragma unroll
@@ -416,27 +438,41 @@ __global__ void __launch_bounds__(NTHREADS, 1)
             fd = (double)f;
             xd = (double)x;
           }
-          rs = fma(fd * tau_s[j0 + j], xd, rs);
+          const double tj = j == 0 ? t01.x : j == 1 ? t01.y : j == 2 ? t23.x : t23.y;
+          if (j & 1)
+            rs2 = fma(fd * tj, xd, rs2);
+          else
+            rs = fma(fd * tj, xd, rs);
         }
       }
+      rs += rs2;
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(b_tempty);
         mbar_arrive(b_eempty);
       }
+      if (dbg) tw[3] += clock64() - t_e0;
       ++tile;
-      if (h2 & F_LAST_PANEL) {  // the two warp sets of a row: second set through shared memory, fixed order
-        if (hs == 1) red[g] = rs;
+      if (h2 & F_LAST_PANEL) {  // the warp sets of a row: sets 1.. through shared memory, summed in a fixed order
+        if (hs > 0) red[(hs - 1) * GB + g] = rs;
         asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
         if (hs == 0) {
           const double sg = sigma[(int64_t)p * GB + g];
-          rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs + red[g], -8 * (2 * NSL + 1));
+#pragma unroll
+          for (int q = 0; q < NSET - 1; ++q) rs += red[q * GB + g];
+          rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs, -8 * (2 * NSL + 1));
         }
         asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
         rs = 0.0;
       }
     }
+  }
+  if (dbg && lane == 0) {  // per role: [0..5] wait slots, [6] lifetime, [7] warps
+    const int role = warp == W_PROD ? 0 : warp == W_MMA ? 1 : warp < W_EPI0 ? 2 : 3;
+    for (int i = 0; i < 6; ++i) atomicAdd(reinterpret_cast<unsigned long long*>(dbg + 8 * role + i), (unsigned long long)tw[i]);
+    atomicAdd(reinterpret_cast<unsigned long long*>(dbg + 8 * role + 6), (unsigned long long)(clock64() - t_begin));
+    atomicAdd(reinterpret_cast<unsigned long long*>(dbg + 8 * role + 7), 1ull);
   }
   tc_fence_before();
   __syncthreads();
@@ -492,10 +528,30 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq);
   KLDI_CUDA(cudaGetLastError());
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  static const bool debug = getenv("KLDI_TC_DEBUG") != nullptr;  // per-role wait cycles, printed to stderr (synchronises)
+  long long* dbg = nullptr;
+  if (debug) {
+    KLDI_CUDA(cudaMalloc(&dbg, 32 * sizeof(long long)));
+    KLDI_CUDA(cudaMemsetAsync(dbg, 0, 32 * sizeof(long long), P->stream));
+  }
   tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phiq, P->d_sigma,
-      P->d_Dq, P->d_tau, n, P->d_rho_s);
+      P->d_Dq, P->d_tau, n, P->d_rho_s, dbg);
   KLDI_CUDA(cudaGetLastError());
+  if (debug) {
+    long long h[32];
+    KLDI_CUDA(cudaStreamSynchronize(P->stream));
+    KLDI_CUDA(cudaMemcpy(h, dbg, sizeof(h), cudaMemcpyDeviceToHost));
+    cudaFree(dbg);
+    const char* names[4] = {"producer [empty, epi_empty]", "mma [hdr, tmem_empty, full_a, full_b]", "gather [hdr]",
+                            "epilogue [hdr, epi_full, tmem_full, compute]"};
+    for (int r = 0; r < 4; ++r) {
+      const double w = (double)h[8 * r + 7];
+      fprintf(stderr, "k_rho_i8 %-46s warps %4.0f life %9.0f waits", names[r], w, h[8 * r + 6] / w);
+      for (int i = 0; i < 4; ++i) fprintf(stderr, " %9.0f", h[8 * r + i] / w);
+      fprintf(stderr, "  (cycles per warp)\n");
+    }
+  }
   return KLDI_OK;
 }
 
