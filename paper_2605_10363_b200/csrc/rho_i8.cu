@@ -12,7 +12,7 @@
 // The digit pairs of equal weight c = i + j accumulate exactly in one int32 TMEM accumulator (|sum| <= K (c+1) 127^2 <
 // 2^31 for K <= 16384), classes c <= NSL-1 are kept (the dropped ones are below 256^-(NSL+1) relative to sigma tau K):
 //     X'(g,n) = sigma_g tau_n 256^-(NSL+1)  sum_c acc_c(g,n) 256^(NSL-1-c)
-// and the epilogue forms rho in FP64 from the int64 recombination and the FP64 Phi store.  NSL = 5: 15 int8 products,
+// and the epilogue forms rho in FP64 from the integer recombination and the FP64 Phi columns of the tile.  NSL = 5: 15 int8 products,
 // max|d rho| ~ 1e-10 on the 8-water case (tolerance 1e-9); NSL = 6: 21 products, ~3e-13.
 #include <cstdio>
 #include <cstdlib>
@@ -28,12 +28,9 @@ constexpr int NT = 96;                       // N-tile width (NSL * NT <= 512 TM
 constexpr int A_SLICE = GB * KC;             // 4096 B: one digit plane of a 128 x 32 Phi chunk
 constexpr int NCH = 2 * (NT / 32);           // gather units of a stage (32 columns x 16 K rows) = gather warps per group
 constexpr int B_SLICE = (NT / 8) * 256;      // 3072 B: one digit plane of a 32 x 96 D' tile
-constexpr int NST = 4;                       // ring stages
+constexpr int NST = 3;                       // ring stages
 constexpr int NGRP = 2;                      // gather groups (alternate stages)
-#ifndef KLDI_TC_NEPI
-#define KLDI_TC_NEPI 16
-#endif
-constexpr int NEPI = KLDI_TC_NEPI;           // epilogue warps: NEPI/4 per TMEM lane quarter, 4-column groups dealt round-robin
+constexpr int NEPI = 8;                      // epilogue warps: NEPI/4 per TMEM lane quarter, 8-column groups dealt round-robin
 constexpr int NSET = NEPI / 4;
 constexpr int W_PROD = 0, W_MMA = 1, W_GATHER0 = 2, W_EPI0 = W_GATHER0 + NGRP * NCH;  // warp roles
 constexpr int NWARPS = W_EPI0 + NEPI;
@@ -43,8 +40,8 @@ enum { F_FIRST = 1, F_LAST_TILE = 2, F_LAST_PANEL = 4, F_DONE = 8 };
 template <int NSL>
 struct Cfg {
   static constexpr int STAGE_BYTES = NSL * (A_SLICE + B_SLICE);
-  static constexpr int OFF_EPI = NST * STAGE_BYTES;                   // digit planes of the tile's own columns (epilogue)
-  static constexpr int EPI_BYTES = (NT / KC) * NSL * A_SLICE;
+  static constexpr int OFF_EPI = NST * STAGE_BYTES;                   // FP64 Phi columns of the tile (epilogue), [NT][128]
+  static constexpr int EPI_BYTES = NT * GB * 8;
   static constexpr int OFF_HDR = OFF_EPI + EPI_BYTES;                 // [NST][4] int
   static constexpr int OFF_KIDX = OFF_HDR + NST * 16;                 // [NST][32] int: plan AO index of the stage's K rows
   static constexpr int OFF_CIDX = OFF_KIDX + NST * KC * 4;            // [4][NT] int: plan AO index of the tile's columns
@@ -111,7 +108,7 @@ __global__ void __launch_bounds__(128) k_slice_phi(const int32_t* __restrict__ t
 __global__ void __launch_bounds__(256) k_colmax(const double* __restrict__ Dp, int n, unsigned long long* __restrict__ mx) {
   const int j = blockIdx.x * 32 + (threadIdx.x & 31);
   const int r0 = blockIdx.y * 256 + (threadIdx.x >> 5);
-  if (j >= n) return;
+  if (j >= n || blockIdx.y * 256 + 255 < blockIdx.x * 32) return;  // rows above the diagonal hold zeros
   double m = 0.0;
   for (int r = r0; r < min(n, blockIdx.y * 256 + 256); r += 8) m = fmax(m, fabs(Dp[(int64_t)r * n + j]));
   if (m > 0.0) atomicMax(mx + j, (unsigned long long)__double_as_longlong(m));
@@ -124,6 +121,7 @@ __global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, 
                                                  double* __restrict__ tau, unsigned long long* __restrict__ Dq) {
   const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y;
   if (j >= n) return;
+  if (blockIdx.x * 256 > i && i > 0) return;  // strictly above the diagonal: Dq was zeroed once and is never written there
   const double m = cmax[j];
   const double t = m > 0.0 ? m * (256.0 / 127.0) : 1.0;
   if (i == 0) tau[j] = t;
@@ -141,27 +139,31 @@ __global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, 
 }
 
 // ------------------------------------------------------------------------------------------------ the contraction
-// Persistent, one CTA per SM, warp-specialised:
+// Persistent, one CTA per SM, warp-specialised (22 warps):
 //   warp 0      scheduler + A producer: pulls grid blocks from the atomic ticket, walks the block's
 //               (N-tile, K-chunk) stages, writes the stage header and the AO indices of the stage's K rows (and, per
-//               tile, of its columns), bulk-copies the chunk's NSL digit planes of Phi, and after the last stage of a
-//               tile the digit planes of the tile's OWN columns into the epilogue buffer
-//   warps 4-15  B builders, two groups of six on alternate stages: warp c of a group gathers the 16 columns
-//               [n0+16c, n0+16c+16) x 32 rows of D' (lane = K row, 16 x 8-byte digit words), transposes the bytes to
-//               digit planes with PRMT and stores them in the MN-major core-matrix layout (NSL x 16-byte stores)
-//   warp 1      MMA issuer: one elected lane issues the NSL(NSL+1)/2 tcgen05.mma of a stage (A_i x B_j -> class i+j)
-//               and commits them to the stage's empty barrier (and to tmem_full after the last chunk of a tile)
-//   warps 16-19 epilogue: TMEM -> registers (one lane = one grid row), int64 recombination of the classes and of the
-//               row's Phi digits (epilogue buffer), FP64 rho += tau_n Phi_int(g,n) X_int(g,n); rho_p at the end of
-//               the panel.  No FP64 Phi is read: the digit planes are the only Phi traffic of the kernel.
+//               tile, of its columns), bulk-copies the chunk's NSL digit planes of Phi (one 20 KB copy), and after the
+//               last stage of a tile the tile's FP64 Phi columns (contiguous in the store: one copy) for the epilogue
+//   warps 2-13  B builders, two groups of six on alternate stages: a warp gathers 32 tile columns x 16 K rows of D'
+//               (lane = column; an instruction reads ONE row of Dq at the ascending AO indices of 32 consecutive packed
+//               columns, a few 128-byte lines), transposes the bytes of the 8-byte digit words to digit planes with PRMT
+//               and stores them K-major (NSL x 16-byte stores, conflict-free)
+//   warp 1      TMEM owner and MMA issuer: one elected lane issues the tcgen05.mma of a stage and commits them to the
+//               stage's empty barrier (and to tmem_full after the last chunk of a tile).  Full-width chunks pair the
+//               digit planes of D' (A_i x [B_j | B_j+1] -> classes i+j, i+j+1: 9 instructions), narrow ones use the
+//               NSL(NSL+1)/2 single products at N = the columns the chunk reaches
+//   warps 14-21 epilogue: TMEM -> registers (one lane = one grid row, two warps per lane quarter on alternate 8-column
+//               groups), integer recombination of the classes, FP64 rho += tau_n Phi(g,n) X_int(g,n) with Phi from the
+//               staged columns; rho_p at the end of the panel (the two warp sets summed in a fixed order)
 // D' is lower triangular in packed order, so only the chunks k0 >= n0 reach tile [n0, n0+Wj) and chunk [k0, k0+32)
 // only its columns n < k0 + 32; the chunks are walked in DESCENDING k0, so the first one is full width and overwrites
-// (zeroes) every accumulator column of the tile.
+// (zeroes) every accumulator column of the tile.  The five accumulator classes of a 96-column tile fill tensor memory
+// (480 of 512 columns), so the MMAs of a tile and the epilogue of the previous one alternate.
 template <int NSL>
 __global__ void __launch_bounds__(NTHREADS, 1)
     k_rho_i8(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket, const int32_t* __restrict__ kp,
              const int64_t* __restrict__ panel_off, const int64_t* __restrict__ chunk_off,
-             const int32_t* __restrict__ colidx, const unsigned char* __restrict__ phiq,
+             const int32_t* __restrict__ colidx, const double* __restrict__ phi, const unsigned char* __restrict__ phiq,
              const double* __restrict__ sigma, const unsigned long long* __restrict__ Dq, const double* __restrict__ tau,
              int n_ao, double* __restrict__ rho_s, long long* __restrict__ dbg) {
   using C = Cfg<NSL>;
@@ -254,12 +256,13 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           __syncwarp();
           ++t;
         }
-        // the digit planes of the tile's own columns for its epilogue (single buffer: wait for the previous epilogue)
+        // the FP64 Phi columns of the tile for its epilogue (single buffer: wait for the previous epilogue); the columns
+        // of a panel are contiguous in the store, so this is ONE bulk copy
         if (tile > 0) twait(1, b_eempty, (tile - 1) & 1);
         if (lane == 0) {
-          const uint32_t bytes = (uint32_t)(Wj / KC) * (NSL * A_SLICE);
+          const uint32_t bytes = (uint32_t)min(Wj, K8 - n0) * (GB * 8);
           mbar_arrive_expect_tx(b_efull, bytes);
-          bulk_g2s(smem_u32(smem + C::OFF_EPI), phiq + (cbase + n0 / KC) * (int64_t)(NSL * A_SLICE), bytes, b_efull);
+          bulk_g2s(smem_u32(smem + C::OFF_EPI), phi + (base + n0) * GB, bytes, b_efull);
         }
         __syncwarp();
       }
@@ -301,12 +304,30 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 #pragma unroll
         for (int q = 1; q < NST; ++q)
           if (s == q) { a = da[q]; b = db[q]; }
+        // Full-width chunks: digit i of Phi against the digits j, j+1 of D' in ONE instruction.  The B planes of a stage
+        // are contiguous and so are the accumulator classes, so A_i x [B_j | B_j+1] (N = 2 NT) adds into the classes i+j
+        // and i+j+1, and the 4 KB A plane is read from shared memory once for two products (9 instructions instead of
+        // 15).  The plane rows beyond the tile width only reach accumulator columns nobody reads.  Narrow (diagonal)
+        // chunks use single planes at N = wact.
+        if (wact == ((h2 >> 16) & 0xff)) {
+          const uint32_t id2 = umma_idesc_s8(2 * NT), id1 = umma_idesc_s8(NT);
 #pragma unroll
-        for (int c = 0; c < NSL; ++c)
+          for (int i = 0; i < NSL; ++i) {
 #pragma unroll
-          for (int i = 0; i <= c; ++i)
-            umma_i8(tmem + c * NT, a + (uint64_t)(i * (A_SLICE >> 4)), b + (uint64_t)((c - i) * (B_SLICE >> 4)), idesc,
-                    i == 0 ? keep : 1u);
+            for (int j = 0; i + j < NSL; j += 2) {
+              const bool two = i + j + 1 < NSL;
+              umma_i8(tmem + (i + j) * NT, a + (uint64_t)(i * (A_SLICE >> 4)), b + (uint64_t)(j * (B_SLICE >> 4)),
+                      two ? id2 : id1, i == 0 ? keep : 1u);
+            }
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < NSL; ++i)
+#pragma unroll
+            for (int j = 0; i + j < NSL; ++j)
+              umma_i8(tmem + (i + j) * NT, a + (uint64_t)(i * (A_SLICE >> 4)), b + (uint64_t)(j * (B_SLICE >> 4)), idesc,
+                      i == 0 ? keep : 1u);
+        }
         umma_commit(b_empty + 8 * s);
         if (h2 & F_LAST_TILE) umma_commit(b_tfull);
       }
@@ -375,12 +396,12 @@ __global__ void __launch_bounds__(NTHREADS, 1)
   } else {
     // ------------------------------------------------------------------ epilogue
     const int qd = warp & 3;                 // TMEM lane quarter of this warp
-    const int hs = (warp - W_EPI0) >> 2;     // warp set: 4-column groups with group % NSET == hs
+    const int hs = (warp - W_EPI0) >> 2;     // warp set: 8-column groups with group % NSET == hs
     const int g = 32 * qd + lane;
     double* tau_s = reinterpret_cast<double*>(smem + C::OFF_TAU) + (warp - W_EPI0) * NT;
     double* red = reinterpret_cast<double*>(smem + C::OFF_RED);
     const uint32_t tl = tmem + ((uint32_t)(32 * qd) << 16);
-    const unsigned char* eg = smem + C::OFF_EPI + (g >> 3) * 256 + (g & 7) * 16;  // this row's 16-byte words
+    const double* ephi = reinterpret_cast<const double*>(smem + C::OFF_EPI) + g;  // this row of the tile's Phi columns
     double rs = 0.0;
     uint32_t tile = 0;
     for (uint32_t t = 0;; ++t) {
@@ -401,48 +422,35 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       tc_fence_after();
       const long long t_e0 = dbg ? clock64() : 0;
       double rs2 = 0.0;
-      for (int j0 = 4 * hs; j0 < wj; j0 += 4 * NSET) {
-        uint32_t dg[NSL];  // digit i of this row for the columns j0 .. j0+3
+      for (int j0 = 8 * hs; j0 < wj; j0 += 8 * NSET) {
+        int32_t acc[NSL][8];
 #pragma unroll
-        for (int i = 0; i < NSL; ++i)
-          dg[i] = *reinterpret_cast<const uint32_t*>(eg + (j0 >> 5) * (NSL * A_SLICE) + i * A_SLICE + ((j0 >> 4) & 1) * 128 +
-                                                     (j0 & 12));
-        int32_t acc[NSL][4];
+        for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
+        double f[8];  // tau_n Phi(g,n) of the columns j0 .. j0+7
 #pragma unroll
-        for (int c = 0; c < NSL; ++c) tmem_ld4(tl + c * NT + j0, acc[c]);
-        const double2 t01 = *reinterpret_cast<const double2*>(tau_s + j0), t23 = *reinterpret_cast<const double2*>(tau_s + j0 + 2);
+        for (int j = 0; j < 8; ++j) f[j] = ephi[(j0 + j) * GB] * tau_s[j0 + j];
         tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          int d[NSL];
-#pragma unroll
-          for (int c = 0; c < NSL; ++c) d[c] = sext_byte(dg[c], j);
-          // Phi_int = sum_c d_c 256^(NSL-1-c), X_int = sum_c acc_c 256^(NSL-1-c): integer parts below 2^51 go to FP64
-          // through the 2^52 + 2^51 mantissa trick (one integer multiply-add chain + one DADD each)
+        for (int j = 0; j < 8; ++j) {
+          // X_int = sum_c acc_c 256^(NSL-1-c) in two integer parts below 2^51, each to FP64 through the 2^52 + 2^51
+          // mantissa trick (an integer multiply-add chain + one DADD)
           constexpr long long MAGIC = 0x4338000000000000LL;
           constexpr double MAGIC_D = 6755399441055744.0;
-          double fd, xd;
+          double xd;
           if (NSL == 5) {
-            const int fh = d[0] * 256 + d[1], fl = (d[2] * 256 + d[3]) * 256 + d[4];
-            fd = __longlong_as_double((long long)fh * 16777216 + ((long long)fl + MAGIC)) - MAGIC_D;
             const long long xh = (long long)acc[0][j] * 65536 + ((long long)acc[1][j] * 256 + ((long long)acc[2][j] + MAGIC));
             const long long xl = (long long)acc[3][j] * 256 + ((long long)acc[4][j] + MAGIC);
             xd = fma(__longlong_as_double(xh) - MAGIC_D, 65536.0, __longlong_as_double(xl) - MAGIC_D);
           } else {
-            long long f = 0, x = 0;
+            long long x = 0;
 #pragma unroll
-            for (int c = 0; c < NSL; ++c) {
-              f = f * 256 + d[c];
-              x = x * 256 + acc[c][j];
-            }
-            fd = (double)f;
+            for (int c = 0; c < NSL; ++c) x = x * 256 + acc[c][j];
             xd = (double)x;
           }
-          const double tj = j == 0 ? t01.x : j == 1 ? t01.y : j == 2 ? t23.x : t23.y;
           if (j & 1)
-            rs2 = fma(fd * tj, xd, rs2);
+            rs2 = fma(f[j], xd, rs2);
           else
-            rs = fma(fd * tj, xd, rs);
+            rs = fma(f[j], xd, rs);
         }
       }
       rs += rs2;
@@ -461,7 +469,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           const double sg = sigma[(int64_t)p * GB + g];
 #pragma unroll
           for (int q = 0; q < NSET - 1; ++q) rs += red[q * GB + g];
-          rho_s[(int64_t)p * GB + g] = 2.0 * sg * sg * scalbn(rs, -8 * (2 * NSL + 1));
+          rho_s[(int64_t)p * GB + g] = 2.0 * sg * scalbn(rs, -8 * (NSL + 1));
         }
         asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
         rs = 0.0;
@@ -501,6 +509,7 @@ static kldi_status tc_prepare(kldi_plan* P) {
   KLDI_CUDA(cudaMalloc(&P->d_sigma, sizeof(double) * P->n_pad));
   KLDI_CUDA(cudaMalloc(&P->d_phiq, (size_t)std::max<int64_t>(1, P->tc_chunks) * NSL * tc::A_SLICE));
   KLDI_CUDA(cudaMalloc(&P->d_Dq, sizeof(unsigned long long) * (size_t)P->n_ao * P->n_ao));
+  KLDI_CUDA(cudaMemsetAsync(P->d_Dq, 0, sizeof(unsigned long long) * (size_t)P->n_ao * P->n_ao, P->stream));
   KLDI_CUDA(cudaMalloc(&P->d_tau, sizeof(double) * 2 * P->n_ao));
   if (P->n_tasks > 0) {
     tc::k_slice_phi<NSL><<<P->n_tasks, 128, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_phi,
@@ -535,8 +544,8 @@ kldi_status launch_rho_tc(kldi_plan* P) {
     KLDI_CUDA(cudaMemsetAsync(dbg, 0, 32 * sizeof(long long), P->stream));
   }
   tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
-      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phiq, P->d_sigma,
-      P->d_Dq, P->d_tau, n, P->d_rho_s, dbg);
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phi, P->d_phiq,
+      P->d_sigma, P->d_Dq, P->d_tau, n, P->d_rho_s, dbg);
   KLDI_CUDA(cudaGetLastError());
   if (debug) {
     long long h[32];
