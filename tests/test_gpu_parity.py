@@ -526,3 +526,131 @@ def test_rho_dfma_option_parity(K, name, n):
     assert E1 == E2 and torch.equal(r1, r2)
     assert float((r1 - r0).abs().max()) <= 1e-12 * max(1.0, float(r0.abs().max()))
     plan.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg0", None), ("cfg1", 8), ("cfg2", 6), ("cfg3", 12), ("cfg1", None)])
+def test_rho_tensor_core_option_parity(K, name, n):
+    """KLDI_OPT_RHO_TC: the LDA rho contraction as int8 slice products on tcgen05 (five base-256
+    digits of Phi and D', 15 exact int32 products, FP64 recombination) — the SAME parity bar against the dense oracle
+    (1e-9 / 1e-9 / 1e-8), rho and E bitwise reproducible, option ignored for GGA; includes cfg1 at full size."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional="lda")
+    plan = K.Plan.from_workload(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    r0 = plan.eval_rho(D).clone()
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+    E1, V1 = plan.exc(D)
+    r1 = plan.eval_rho(D).clone()
+    E2, _ = plan.exc(D)
+    r2 = plan.eval_rho(D)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda")
+    check({"rho": r1.cpu().numpy(), "V": V1.cpu().numpy(), "E": E1, "drho": None}, ref)
+    assert E1 == E2 and torch.equal(r1, r2)
+    # the digit truncation is visible against the FP64 path but far inside the bar
+    assert float((r1 - r0).abs().max()) <= 2e-10
+    plan.close()
+
+
+def test_rho_tensor_core_option_edge_cases(K):
+    """Ragged shapes through the tcgen05 path: a single point, 129 points, a minimal basis (K_p = 1 -> one padded chunk),
+    an empty plan; and a D with entries of very different magnitude per column (the column scale tau_n)."""
+    import torch
+
+    wl = W.named_config("cfg0")
+    basis = basis_of(wl)
+    D = torch.as_tensor(wl.D, device="cuda")
+    for n in (1, 129):
+        pts, w = wl.grid_xyz[2000:2000 + n], wl.grid_w[2000:2000 + n]
+        plan = K.Plan(*basis, pts, w, 1e-12)
+        plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+        ref = O.exc(basis, pts, w, wl.D, "lda")
+        assert np.max(np.abs(plan.eval_rho(D).cpu().numpy() - ref["rho"])) <= TOL_RHO
+        plan.close()
+    far = wl.grid_xyz[:300] + 500.0
+    plan = K.Plan(*basis, far, wl.grid_w[:300], 1e-12)
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+    assert float(plan.eval_rho(D).abs().max()) == 0.0
+    plan.close()
+    one = (np.zeros((1, 3)), np.array([0], np.int32), np.array([0], np.int32), np.array([0, 1], np.int32),
+           np.array([0.9]), np.array([1.0]))
+    pts, w = W.atomic_grid(1.0)
+    plan = K.Plan(*one, pts, w, 1e-12)
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+    rho = plan.eval_rho(torch.tensor([[2.0]], dtype=torch.float64, device="cuda")).cpu().numpy()
+    ref = O.exc(one, pts, w, np.array([[2.0]]), "lda")
+    assert np.max(np.abs(rho - ref["rho"])) <= 1e-10
+    plan.close()
+    # columns of D scaled by powers of ten (symmetrised): every column keeps its own 40 bits
+    wl8 = W.named_config("cfg1", n_override=4)
+    s = 10.0 ** np.random.default_rng(5).integers(-6, 1, wl8.n_ao)
+    Ds = wl8.D * np.sqrt(s[:, None] * s[None, :])
+    plan = K.Plan.from_workload(wl8)
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+    rho = plan.eval_rho(torch.as_tensor(Ds, device="cuda")).cpu().numpy()
+    ref = O.exc(basis_of(wl8), wl8.grid_xyz, wl8.grid_w, Ds, "lda", want_v=False)
+    assert np.max(np.abs(rho - ref["rho"])) <= TOL_RHO
+    plan.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_parity_full_size_elementwise(K, name):
+    """BASELINE.json configs[2] (C60H122, 1,510 AOs, 1,001,000 points) and configs[4] (64 waters, GGA) at FULL size
+    against the dense oracle, element by element: rho, grad rho, V and E at the north_star tolerances."""
+    wl = W.named_config(name)
+    out = run_gpu(K, wl, deterministic_v=2)
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, wl.functional, chunk=16384)
+    check(out, ref)
+    out["plan"].close()
+
+
+def test_parity_cfg3_full_size_against_golden(K):
+    """BASELINE.json configs[3] (256 waters, 6,400 AOs, 4,224,000 points) at FULL size against the stored result of the
+    dense CPU oracle (tests/golden/cfg3_oracle.npz, written by tests/golden/make_cfg3_golden.py from oracle/ alone):
+    E_xc to 1e-8 Ha, rho on every 64th point and 16 full rows + a strided sample of V to 1e-9 — for the FP64 DMMA
+    path and for the tcgen05 slice-product path, in the launch configuration bench.py times."""
+    import os
+
+    import torch
+
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg3_oracle.npz")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/cfg3_oracle.npz not generated yet (tests/golden/make_cfg3_golden.py)")
+    g = np.load(path)
+    wl = W.named_config("cfg3")
+    assert wl.n_pts == int(g["n_pts"]) and wl.n_ao == int(g["n_ao"])
+    # same inputs: the Becke weights of this run agree with those the golden was computed on to rounding
+    assert abs(wl.grid_w.sum() - float(g["w_sum"])) <= 1e-9 * abs(float(g["w_sum"]))
+    plan = K.Plan.from_workload(wl)
+    plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 2)
+    D = torch.as_tensor(wl.D, device="cuda")
+    sp, (sv0, sv1) = int(g["stride_pts"]), (int(g["stride_v"][0]), int(g["stride_v"][1]))
+    rows = [int(r) for r in g["v_rows"]]
+    for tc in (0, 1):
+        plan.set_option(K.KLDI_OPT_RHO_TC, tc)
+        E, V = plan.exc(D)
+        rho = plan.eval_rho(D).cpu().numpy()
+        V = V.cpu().numpy()
+        assert abs(E - float(g["E"])) <= TOL_E, (tc, E, float(g["E"]))
+        assert np.max(np.abs(rho[::sp] - g["rho_strided"])) <= TOL_RHO
+        assert np.max(np.abs(V[rows, :] - g["V_rows"])) <= TOL_V
+        assert np.max(np.abs(V[::sv0, ::sv1] - g["V_strided"])) <= TOL_V
+        assert np.array_equal(V, V.T)
+    plan.close()
+
+
+def test_becke_cuda_equals_numpy():
+    """Input generation only: the CUDA Becke helper (workloads/becke.cu) reproduces the numpy recipe it stands in for
+    (plain Becke, 3 smoothing iterations) on a 9-atom case, to rounding."""
+    from paper_2605_10363_b200.workloads import generate as G
+
+    symbols, xyz = G.water_cluster_geometry(3, 77)
+    pts, w, owner = [], [], []
+    for ia, s in enumerate(symbols):
+        p, ww = G.atomic_grid(G._RADIAL_SCALE[s])
+        pts.append(p + xyz[ia]); w.append(ww); owner.append(np.full(p.shape[0], ia, np.int32))
+    pts, owner = np.vstack(pts), np.concatenate(owner)
+    a = G.becke_weights(xyz, pts, owner, backend="cuda")
+    b = G.becke_weights(xyz, pts, owner, backend="numpy")
+    assert a.shape == b.shape and np.max(np.abs(a - b)) <= 1e-12
+    assert 0.0 <= a.min() and a.max() <= 1.0 + 1e-15
