@@ -94,8 +94,6 @@ class ClockSampler:
 
 def cpu_oracle_sample(wl, n_sample: int):
     """The oracle as it stands on a bounded, strided sample of the workload's grid points."""
-    import torch
-
     from oracle import exc_oracle as O
 
     idx = np.arange(0, wl.n_pts, max(1, wl.n_pts // n_sample))[:n_sample]
@@ -107,7 +105,13 @@ def cpu_oracle_sample(wl, n_sample: int):
         cores = len(os.sched_getaffinity(0))
     except AttributeError:
         cores = os.cpu_count()
-    return {"value": evals_per_s, "unit": UNIT, "cores": min(cores, torch.get_num_threads()) if cores else None,
+    try:                                   # the oracle is numpy: its dgemm threads are the BLAS pool's
+        from threadpoolctl import threadpool_info
+        blas = [int(p["num_threads"]) for p in threadpool_info() if p.get("user_api") == "blas"]
+        cores = min(cores, max(blas)) if blas and cores else cores
+    except Exception:
+        pass
+    return {"value": evals_per_s, "unit": UNIT, "cores": cores,
             "kind": "oracle",
             "sample": f"every {max(1, wl.n_pts // n_sample)}-th grid point ({len(idx)} of {wl.n_pts}), dense, "
                       f"{dt:.1f} s, extrapolated linearly in n_pts"}, dt
@@ -155,8 +159,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pair-test", type=int, default=0, choices=[0, 1],
                     help="1: executable-pair selection a_pq*b_qr >= eps per call (Eq. 17-19)")
-    ap.add_argument("--deterministic-v", type=int, default=0, choices=[0, 1, 2],
-                    help="V without FP64 atomics: 1 = workspace partials + fixed-order reduce, 2 = fixed-point integer atomics")
+    ap.add_argument("--deterministic-v", type=int, default=2, choices=[0, 1, 2],
+                    help="V accumulation: 2 (library default) = fixed-point integer atomics, bitwise reproducible; "
+                         "1 = workspace partials + fixed-order reduce; 0 = FP64 atomics")
+    ap.add_argument("--rho-tc", type=int, default=0, choices=[0, 1],
+                    help="1: headline step with the tcgen05 int8 slice-product rho contraction (KLDI_OPT_RHO_TC); "
+                         "0 times it as the extra leg tensor_core_rho")
     ap.add_argument("--rho-dfma", type=int, default=0, choices=[0, 1],
                     help="1: LDA rho contraction on the vector FP64 pipe (register tiles) instead of DMMA tiles")
     ap.add_argument("--grad", action="store_true",
@@ -194,13 +202,15 @@ def main():
     gen_s = time.perf_counter() - t0
     wl = wl_full
     if world > 1:
-        wl, _ = sharding.shard_workload(wl_full, rank, world)
+        wl, _ = sharding.shard_workload(wl_full, rank, world)     # cost-balanced range of the plan's curve order
     gga = wl.functional == "gga"
     func = K.KLDI_GGA_PBEX if gga else K.KLDI_LDA_SLATER
     plan = K.Plan.from_workload(wl)
     plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
     plan.set_option(K.KLDI_OPT_PAIR_TEST, args.pair_test)
     plan.set_option(K.KLDI_OPT_RHO_DFMA, args.rho_dfma)
+    if not gga:
+        plan.set_option(K.KLDI_OPT_RHO_TC, args.rho_tc)
     st = plan.stats.as_dict()
     D = torch.as_tensor(wl.D, device="cuda")
     V = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")
@@ -222,12 +232,16 @@ def main():
         ev0.record()
         for _ in range(args.steps):
             E = step()
-            for k, v in plan.last_timings().items():
-                stage_ms[k] = stage_ms.get(k, 0.0) + v / args.steps
         ev1.record()
         torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
+    n_stage = min(args.steps, 10)          # per-stage times from the library's own CUDA events: a separate, untimed pass
+    for _ in range(n_stage):
+        step()
+        for k, v in plan.last_timings().items():
+            stage_ms[k] = stage_ms.get(k, 0.0) + v / n_stage
+    launches = int(plan.refresh_stats().kernel_launches)
     ms = ev0.elapsed_time(ev1)
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
@@ -236,56 +250,105 @@ def main():
     ms_per_step = ms / args.steps
     value = 1e3 / ms_per_step
 
-    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of D and D2H of V inside the timed region
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of D and D2H of V inside the timed region.
+    # D and V are symmetric: kldi_exc_host uploads the lower triangle of D, and with KLDI_OPT_HOST_V_TRIANGLE it
+    # downloads only the lower triangle of V (row bands); the full-matrix download is timed beside it.
     e2e = None
     if world == 1:
         Dh = torch.as_tensor(wl.D).pin_memory()
         Vh = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64).pin_memory()
-        for _ in range(2):
-            plan.exc_host(Dh, func, Vh)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            plan.exc_host(Dh, func, Vh)
-        torch.cuda.synchronize()
-        e2e_s = (time.perf_counter() - t0) / args.steps
         nn = wl.n_ao * wl.n_ao * 8
-        bands = 1 if wl.n_ao < 1024 else 32           # kldi_exc_host uploads the lower triangle of D in row bands
-        h2d = sum(8 * (wl.n_ao * (b + 1) // bands) * (wl.n_ao * (b + 1) // bands - wl.n_ao * b // bands)
+        bands = 1 if wl.n_ao < 1024 else 32
+        tri = sum(8 * (wl.n_ao * (b + 1) // bands) * (wl.n_ao * (b + 1) // bands - wl.n_ao * b // bands)
                   for b in range(bands))
-        e2e = {"value": 1.0 / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": nn + 8,
-               "ms_per_step": e2e_s * 1e3}
+        res = {}
+        for mode in (1, 0):
+            plan.set_option(K.KLDI_OPT_HOST_V_TRIANGLE, mode)
+            for _ in range(2):
+                plan.exc_host(Dh, func, Vh)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                plan.exc_host(Dh, func, Vh)
+            torch.cuda.synchronize()
+            res[mode] = (time.perf_counter() - t0) / args.steps
+        plan.set_option(K.KLDI_OPT_HOST_V_TRIANGLE, 0)
+        e2e = {"value": 1.0 / res[1], "unit": UNIT, "h2d_bytes_per_step": tri, "d2h_bytes_per_step": tri + 8,
+               "ms_per_step": res[1] * 1e3, "mode": "lower triangles of D (upload) and V (download), row bands",
+               "full_v_download": {"value": 1.0 / res[0], "ms_per_step": res[0] * 1e3, "d2h_bytes_per_step": nn + 8}}
 
-    # ---- the same step with the bitwise-reproducible V accumulation (64-bit fixed-point integer atomics)
-    fx_leg = None
-    if world == 1 and args.deterministic_v == 0:
-        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 2)
+    # ---- the same step with the other V accumulation mode (0 = FP64 atomics; the default 2 = 64-bit fixed-point
+    # integer atomics, bitwise reproducible) and, for LDA, with the tcgen05 int8 slice-product rho contraction
+    def timed_leg(n):
         for _ in range(3):
             plan.exc(D, func, out=V)
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         f0.record()
-        for _ in range(args.steps):
+        for _ in range(n):
             plan.exc(D, func, out=V)
         f1.record()
         torch.cuda.synchronize()
+        return 1e3 * n / f0.elapsed_time(f1)
+
+    fx_leg, tc_leg = None, None
+    if world == 1:
+        other = 0 if args.deterministic_v == 2 else 2
         Va = V.clone()
         plan.exc(D, func, out=V)
-        fx_leg = {"mode": "KLDI_OPT_DETERMINISTIC_V=2 (fixed-point integer atomics, no FP64 atomics)",
-                  "evals_per_s": 1e3 * args.steps / f0.elapsed_time(f1), "vxc_ms": plan.last_timings()["vxc"],
-                  "bitwise_equal_between_calls": bool(torch.equal(Va, V))}
-        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, 0)
+        same = bool(torch.equal(Va, V))
+        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, other)
+        fx_leg = {"headline_mode": args.deterministic_v, "headline_bitwise_equal_between_calls": same,
+                  "other_mode": other, "other_mode_evals_per_s": timed_leg(args.steps),
+                  "other_mode_vxc_ms": plan.last_timings()["vxc"],
+                  "modes": "2 = fixed-point integer atomics (no FP64 atomics, reproducible), 0 = red.global.add.f64"}
+        plan.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
+    if world == 1 and not gga:
+        rho_ref = plan.eval_rho(D).clone()
+        plan.set_option(K.KLDI_OPT_RHO_TC, 1 - args.rho_tc)
+        evs = timed_leg(args.steps)
+        tms = plan.last_timings()
+        st_tc = plan.refresh_stats().as_dict()
+        rho_tc = plan.eval_rho(D)
+        which = "KLDI_OPT_RHO_TC=%d" % (1 - args.rho_tc)
+        tc_leg = {"option": which, "evals_per_s": evs, "rho_ms": tms["rho"], "total_ms": tms["total"],
+                  "max_abs_d_rho_between_paths": float((rho_tc - rho_ref).abs().max()),
+                  "int8_ops_per_launch": st_tc["ops_rho_tc"], "kernel_launches": st_tc["kernel_launches"]}
+        plan.set_option(K.KLDI_OPT_RHO_TC, args.rho_tc)
+        del rho_ref, rho_tc
 
-    # ---- BASELINE.json configs[3]: how the retained fraction, the throughput and the result move with eps.  The
-    # differences are taken against this run's eps (GPU vs GPU: the screening increment; oracle parity is in tests/).
+    # ---- BASELINE.json configs[3]: how the retained fraction, the throughput and the result move with eps.  The three
+    # errors are taken against the stored result of the dense CPU oracle (tests/golden/cfg3_oracle.npz, written from
+    # oracle/ alone): E_xc, rho on every 64th point, 16 full rows + a strided sample of V; without the file, against
+    # this run's eps = 1e-12 result (GPU vs GPU: the screening increment only).
     eps_leg = None
+    second_plan_s = None
     if world == 1 and args.config == "cfg3" and abs(args.eps - 1e-12) < 1e-20:
+        gpath = os.path.join(ROOT, "tests", "golden", "cfg3_oracle.npz")
+        gold = np.load(gpath) if os.path.exists(gpath) else None
         rho_a = plan.eval_rho(D).clone()
         Ea, _ = plan.exc(D, func, out=V)
         Va = V.clone()
-        eps_leg = []
+
+        def errors(E_, rho_, V_):
+            if gold is not None:
+                sp, sv = int(gold["stride_pts"]), gold["stride_v"]
+                rows = torch.as_tensor(gold["v_rows"], device="cuda")
+                return {"reference": "dense CPU oracle (tests/golden/cfg3_oracle.npz)",
+                        "max_abs_d_rho": float((rho_[::sp].cpu() - torch.as_tensor(gold["rho_strided"])).abs().max()),
+                        "max_abs_d_V": max(float((V_[rows].cpu() - torch.as_tensor(gold["V_rows"])).abs().max()),
+                                           float((V_[::int(sv[0]), ::int(sv[1])].cpu() - torch.as_tensor(gold["V_strided"])).abs().max())),
+                        "abs_d_E": abs(E_ - float(gold["E"]))}
+            return {"reference": "this run at eps = 1e-12 (GPU vs GPU)",
+                    "max_abs_d_rho": float((rho_ - rho_a).abs().max()), "max_abs_d_V": float((V_ - Va).abs().max()),
+                    "abs_d_E": abs(E_ - Ea)}
+
+        eps_leg = [dict(eps=args.eps, evals_per_s=value, **errors(Ea, rho_a, Va))]
         for eps2 in (1e-10, 1e-8):
             p2 = K.Plan.from_workload(wl, eps=eps2)
+            p2.set_option(K.KLDI_OPT_DETERMINISTIC_V, args.deterministic_v)
+            if eps2 == 1e-10:
+                second_plan_s = p2.stats.plan_seconds      # a plan after the first of the process: no module loading
             V2 = torch.empty_like(V)
             for _ in range(3):
                 E2, _ = p2.exc(D, func, out=V2)
@@ -297,13 +360,11 @@ def main():
             q1.record()
             torch.cuda.synchronize()
             s2 = p2.stats.as_dict()
-            eps_leg.append({"eps": eps2, "evals_per_s": 5e3 / q0.elapsed_time(q1),
-                            "retained_blocks_over_candidates": s2["retained_blocks"] / s2["candidate_blocks"],
-                            "sum_k": s2["sum_k"], "phi_bytes": s2["phi_bytes"],
-                            "retained_over_dense_flops": (s2["flops_rho_useful_sym"] + s2["flops_v_useful"]) / (2 * s2["flops_dense"]),
-                            "max_abs_d_rho_vs_eps1e-12": float((p2.eval_rho(D) - rho_a).abs().max()),
-                            "max_abs_d_V_vs_eps1e-12": float((V2 - Va).abs().max()),
-                            "abs_d_E_vs_eps1e-12": abs(E2 - Ea)})
+            eps_leg.append(dict(eps=eps2, evals_per_s=5e3 / q0.elapsed_time(q1),
+                                retained_blocks_over_candidates=s2["retained_blocks"] / s2["candidate_blocks"],
+                                sum_k=s2["sum_k"], phi_bytes=s2["phi_bytes"],
+                                retained_over_dense_flops=(s2["flops_rho_useful_sym"] + s2["flops_v_useful"]) / (2 * s2["flops_dense"]),
+                                **errors(E2, p2.eval_rho(D), V2)))
             p2.close()
         del rho_a, Va
 
@@ -387,14 +448,29 @@ def main():
                          "flops_per_launch": f_v, "exec_flops_per_launch": st["flops_v_exec"],
                          "exec_frac": st["flops_v_exec"] / (stage_ms["vxc"] * 1e-3) / 1e12 / fp64_clock_peak,
                          "schedule_critical_path_flops": st["flops_v_crit"],
-                         "deterministic": bool(args.deterministic_v)}}
-    tr = os.path.join(ROOT, "profiles", "traffic.csv")  # ncu --set full DRAM bytes per launch (text, committed)
+                         "accumulation_mode": args.deterministic_v}}
+    # DRAM bytes per launch come from an `ncu --set full` capture, which cannot run inside a timed benchmark: the
+    # committed text file profiles/traffic.csv (config, kernel, bytes, round, source) is looked up and its provenance
+    # reported; a kernel changed since that capture is the summary's to say.
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")
+    kern = "k_rho_i8" if (args.rho_tc and not gga) else "k_rho"
     if os.path.exists(tr):
         with open(tr) as f:
             for ln in f:
                 c = ln.strip().split(",")
-                if len(c) >= 3 and c[0] == args.config and c[1] == "k_rho" and abs(args.eps - 1e-12) < 1e-20:
+                if len(c) >= 3 and c[0] == args.config and c[1] == kern and abs(args.eps - 1e-12) < 1e-20:
                     roof["traffic"] = int(c[2])
+                    roof["traffic_source"] = "profiles/traffic.csv: " + ", ".join(c[3:])
+    if args.rho_tc and not gga:
+        # tensor-core path: int8 operations issued against the int8 peak (measured bf16 peak x the nominal 2:1 ratio)
+        i8_peak = pk["bf16_tflops"] * 2.0
+        ops = plan.refresh_stats().ops_rho_tc
+        roof.update({"kernel": "k_rho_i8 (rho contraction, tcgen05 kind::i8 slice products)", "unit": "TOP/s (int8)",
+                     "achieved": ops / t_rho / 1e12, "peak": i8_peak, "frac": ops / t_rho / 1e12 / i8_peak,
+                     "peak_source": f"int8 tensor peak = measured bf16 {pk['bf16_tflops']} TFLOP/s ({pk['_source']}) x 2 "
+                                    "(nominal 4.5 : 2.25 PFLOP/s)",
+                     "retained_block_fp64_equivalent_tflops": f_rho / t_rho / 1e12,
+                     "launch_ms_includes": "k_colmax + k_slice_D (D' digits) + k_rho_i8"})
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
@@ -411,13 +487,17 @@ def main():
                   "rho_exec": f_rho_exec, "v_exec": st["flops_v_exec"], "rho_symmetry_halving": not gga,
                   "dense_one_product": st["flops_dense"], "retained_over_dense": f_total / (2 * st["flops_dense"]),
                   "v_symmetry_halving": not gga, "ao_partition": "one AO block per shell"},
-        "stage_ms": stage_ms, "plan_create_s": st["plan_seconds"], "workload_gen_s": gen_s, "exc_energy": E,
+        "stage_ms": stage_ms, "plan_create_s": st["plan_seconds"], "plan_create_note": "first plan of the process (includes one-time module loading)", "workload_gen_s": gen_s, "exc_energy": E,
         "plan": {k: st[k] for k in ("n_blocks", "n_blocks_nonempty", "retained_blocks", "candidate_blocks", "sum_k",
                                      "max_k", "phi_bytes")},
         "pair_test": {"enabled": bool(args.pair_test), "stages_total": plan.refresh_stats().pair_stages_total,
                       "stages_executed": plan.stats.pair_stages_executed},
-        "gpu_launches": 6 + (1 if gga else 0) + {0: 0, 1: 1, 2: 2}[args.deterministic_v] + 2 * args.pair_test, "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
-        "nuclear_gradient": grad_leg, "reproducible_v": fx_leg, "eps_scaling": eps_leg,
+        "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
+        "gpu_launches_note": "kernels of libkldi per kldi_exc, counted by the library (kldi_stats.kernel_launches); "
+                             "the 4-5 cudaMemsetAsync nodes per call are not kernels of this library",
+        "clocks": cs.summary(), "roofline": roof, "e2e": e2e,
+        "nuclear_gradient": grad_leg, "v_accumulation": fx_leg, "tensor_core_rho": tc_leg, "eps_scaling": eps_leg,
+        "plan_create_second_plan_s": second_plan_s,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_oracle_sample(wl_full, args.ref_sample)

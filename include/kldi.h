@@ -11,8 +11,9 @@
  * restricted to the block pairs that survive the block-level filter max|Phi_pq| >= eps
  * (Eq. 11-14) and the executable-pair test a_pq*b_qr >= eps (Eq. 17-19,
  * PAPER.md:195-216), stored in row- and column-oriented block-compressed layouts (BCS(R)/BCS(C),
- * PAPER.md:176-191, 459-471).  A "grid block" p is 128 consecutive points of the Morton-sorted
- * grid (Eq. 20); an "AO block" q is one shell (AO-shell partition).
+ * PAPER.md:176-191, 459-471).  A "grid block" p is 128 consecutive points of the grid sorted along a
+ * space-filling curve (the Hilbert index of Eq. 20's lattice coordinates; kldi_grid_key); an "AO
+ * block" q is one shell (AO-shell partition).
  *
  * Conventions (all calls):
  *   - "host" pointers are ordinary CPU memory; "dev" pointers are CUDA device memory on the
@@ -21,7 +22,7 @@
  *   - AO order at the boundary: shells in the order given, Cartesian components in the order
  *     s | x,y,z | xx,xy,xz,yy,yz,zz; every component is individually normalised (<chi|chi> = 1
  *     for an uncontracted shell with coef = 1).  Grid order: the caller's.  Every internal
- *     permutation (Morton order of points, spatial order of atoms/shells) is undone before
+ *     permutation (curve order of points, spatial order of atoms/shells) is undone before
  *     results are written.
  *   - Matrices are row-major, FP64.  D must be symmetric.
  *   - All work is enqueued on the CUDA stream given to kldi_plan_create.  Calls are
@@ -101,9 +102,11 @@ typedef struct {
   double flops_v_crit;         /* V kernel: 4 scheduler partitions x the busiest partition's units per pass, summed (schedule imbalance) */
   int64_t pair_stages_total;   /* KLDI_OPT_PAIR_TEST, last rho call: (K chunk, N tile) stages before the test; -1 = off */
   int64_t pair_stages_executed;/* ... and stages that contain an executable pair a_pq*b_qr >= eps (Eq. 17-19) */
+  int64_t kernel_launches;     /* kernels of this library launched by the most recent compute call on the plan */
+  double ops_rho_tc;           /* KLDI_OPT_RHO_TC: int8 operations (2 per multiply-add) one rho build issues on the tensor cores */
 } kldi_stats;
 
-/* Once per geometry: Morton reorder of the grid into blocks of 128 (Eq. 20), spatial
+/* Once per geometry: space-filling-curve reorder of the grid into blocks of 128 (Eq. 20's lattice), spatial
  * order of atoms and the AO-shell partition, AO evaluation on candidate (grid block, shell) tiles,
  * block-max filter (keep iff max|chi| >= eps, Eq. 12; with want_gradients the max also runs over the
  * three gradient components), BCS(R)/BCS(C) layouts, task lists.  eps <= 0 retains every block
@@ -154,8 +157,9 @@ kldi_status kldi_last_timings(kldi_plan* plan, double* out);
  *   5 pos          [retained]     BCS(C) -> BCS(R) position of the same block
  *   6 shell_perm   [n_shells]     caller shell index of plan shell q
  *   7 ao_perm      [n_ao]         caller AO index of plan AO i
- *   8 morton_keys  [n_blocks*128] uint64, sorted keys (padding = 2^63)
- *   9 block_amax   [retained]     float64, a_pq = max|Phi_pq| in BCS(R) order
+ *   8 grid_keys    [n_blocks*128] uint64, sorted kldi_grid_key values (padding = 2^63)
+ *   9 block_amax   [retained]     float64, a_pq = max|Phi_pq| in BCS(R) order (with want_gradients the max also runs
+ *                                 over the three gradient tiles, the filter's quantity)
  *  10 panel_off    [n_blocks+1]   int64, first packed column of grid block p in the Phi store
  *  11 blk_col0     [retained]     packed column (within its panel) where the block starts       */
 kldi_status kldi_plan_export(const kldi_plan* plan, int which, void* buf, int64_t cap_bytes,
@@ -190,14 +194,14 @@ kldi_status kldi_build_vtau(kldi_plan* plan, const double* wv_tau, double* V);
 kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, double* Exc, double* grad);
 
 /* Options of a plan (kldi_plan_set_option returns KLDI_EINVAL for an unknown option).
- * KLDI_OPT_DETERMINISTIC_V: 0 (default) = the V contraction adds each grid block's Gram tile into V with
- * red.global.add.f64 (order-dependent rounding, ~1e-16 relative); 1 = the tiles go to a workspace (allocated on
- * first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed order: no FP64 atomics, V bitwise
- * reproducible; 2 = as 0, but every contribution is added as a 64-bit fixed-point integer
- * (red.global.add.u64): integer addition is associative, so V is bitwise reproducible at the speed of mode 0.  The
- * scale is the power of two that keeps every partial sum below 2^61, from a per-call bound
- * max_q sum_p (sum_{g in p} |wv_g|) a_pq^2 >= |V_ij| (Eq. 11 block maxima a_pq; Cauchy-Schwarz); a contribution is
- * rounded once, to 2^-61 of that bound, and the sum itself is exact.  Other values -> KLDI_EINVAL.
+ * KLDI_OPT_DETERMINISTIC_V: how the V contraction adds each grid block's Gram tile into V.  2 (default) = every
+ * contribution is added as a 64-bit fixed-point integer (red.global.add.u64): integer addition is associative, so V is
+ * bitwise reproducible and no FP64 atomic is used; the scale is the power of two that keeps every partial sum below
+ * 2^61, from a per-call bound max_q sum_p (sum_{g in p} |wv_g|) a_pq^2 >= |V_ij| (Eq. 11 block maxima a_pq;
+ * Cauchy-Schwarz); a contribution is rounded once, to 2^-61 of that bound, and the sum itself is exact.  0 =
+ * red.global.add.f64 (order-dependent rounding, ~1e-16 relative; 2 % faster).  1 = the tiles go to a workspace
+ * (allocated on first use, about 4 n_blocks K_p^2 bytes) and are summed per AO row in a fixed order, the per-AO-block
+ * reduction of PAPER.md:222 (bitwise reproducible, several times slower).  Other values -> KLDI_EINVAL.
  * KLDI_OPT_PAIR_TEST: 0 (default) = the rho contraction executes every retained pair (E = I, the conservative
  * superset); 1 = per call, b_qr = max|D_qr| is formed for every AO-shell pair and a (32-column K chunk, N tile)
  * stage of the rho kernel runs only if it contains a pair with a_pq * b_qr >= eps (Eq. 17-19, t_d = eps); costs
@@ -214,8 +218,12 @@ kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, d
  * >= 256^-6 are accumulated exactly, and rho is recombined in FP64.  Error ~1e-10 absolute on rho (same parity bar,
  * 1e-9); rho stays bitwise reproducible.  Costs a second store of 5 bytes per retained Phi value and n_ao^2 64-bit
  * words.  Ignored for GGA, while KLDI_OPT_PAIR_TEST is on, and by kldi_eval_tau / kldi_exc_grad; KLDI_ESTATE from the
- * compute call if a grid block retains more than 16384 AO columns. */
-typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2, KLDI_OPT_RHO_DFMA = 3, KLDI_OPT_RHO_TC = 4 } kldi_option;
+ * compute call if a grid block retains more than 16384 AO columns.
+ * KLDI_OPT_HOST_V_TRIANGLE: 0 (default) = kldi_exc_host fills all of V_host; 1 = only its lower triangle (row >= column,
+ * the convention D is read in), in row bands: V is exactly symmetric, so the other half is redundant and the
+ * device-to-host copy halves. */
+typedef enum { KLDI_OPT_DETERMINISTIC_V = 1, KLDI_OPT_PAIR_TEST = 2, KLDI_OPT_RHO_DFMA = 3, KLDI_OPT_RHO_TC = 4,
+               KLDI_OPT_HOST_V_TRIANGLE = 5 } kldi_option;
 kldi_status kldi_plan_set_option(kldi_plan* plan, kldi_option option, int value);
 
 /* FP64 tensor-pipe microbenchmark: every SM issues dependent-free DMMA.8x8x4 for `iters`
@@ -233,6 +241,9 @@ uint64_t kldi_morton_key(const double* xyz, const double* origin);
  * §8(f1): no jumps along the curve, so blocks of 128 consecutive points are more compact than with the Z-order and
  * retain fewer AO shells.  The order is internal; results do not depend on it.  xyz, origin: HOST [3]. */
 uint64_t kldi_grid_key(const double* xyz, const double* origin);
+/* The same key for n points at once (host only): xyz HOST [n][3], keys HOST [n].  Used by the multi-GPU partition
+ * (contiguous ranges of the plan's curve order). */
+kldi_status kldi_grid_keys(const double* xyz, int64_t n, const double* origin, uint64_t* keys);
 
 /* Host only, no GPU needed: the V-contraction schedule the plan builds for a packed panel of nb column blocks
  * of 8 (square = 0: LDA, strips on and above the diagonal; 1: GGA, full square).  passes: [cap][8] int32

@@ -21,13 +21,14 @@ KLDI_GGA_PBEX = 1
 EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_exc_grad", "kldi_eval_tau", "kldi_build_vtau", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
-    "kldi_morton_key", "kldi_grid_key", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
+    "kldi_morton_key", "kldi_grid_key", "kldi_grid_keys", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
     "kldi_vlayout_offset",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
 KLDI_OPT_PAIR_TEST = 2
 KLDI_OPT_RHO_DFMA = 3
 KLDI_OPT_RHO_TC = 4
+KLDI_OPT_HOST_V_TRIANGLE = 5
 
 
 class KldiError(RuntimeError):
@@ -57,6 +58,7 @@ class Stats(C.Structure):
         ("flops_v_exec", C.c_double), ("flops_dense", C.c_double), ("plan_seconds", C.c_double), ("eps", C.c_double),
         ("flops_rho_useful_sym", C.c_double), ("flops_rho_exec_sym", C.c_double), ("flops_v_crit", C.c_double),
         ("pair_stages_total", C.c_int64), ("pair_stages_executed", C.c_int64),
+        ("kernel_launches", C.c_int64), ("ops_rho_tc", C.c_double),
     ]
 
     def as_dict(self) -> dict:
@@ -95,6 +97,7 @@ def lib():
         L.kldi_morton_key.restype = C.c_uint64
         L.kldi_grid_key.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.kldi_grid_key.restype = C.c_uint64
+        L.kldi_grid_keys.argtypes = [C.c_void_p, C.c_int64, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.kldi_vsched_export.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_vlayout_offset.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
@@ -118,7 +121,7 @@ def _np(a, dtype):
 _EXPORT_DTYPES = {0: np.int32, 1: np.int32, 2: np.int32, 3: np.int32, 4: np.int32, 5: np.int32, 6: np.int32,
                   7: np.int32, 8: np.uint64, 9: np.float64, 10: np.int64, 11: np.int32}
 EXPORT_NAMES = {"perm_g": 0, "row_ptr": 1, "col_idx": 2, "col_ptr": 3, "row_idx": 4, "pos": 5, "shell_perm": 6,
-                "ao_perm": 7, "morton_keys": 8, "block_amax": 9, "panel_off": 10, "blk_col0": 11}
+                "ao_perm": 7, "grid_keys": 8, "morton_keys": 8, "block_amax": 9, "panel_off": 10, "blk_col0": 11}
 
 
 class Plan:
@@ -297,6 +300,15 @@ def grid_key(xyz, origin) -> int:
     a = (C.c_double * 3)(*[float(v) for v in xyz])
     o = (C.c_double * 3)(*[float(v) for v in origin])
     return int(lib().kldi_grid_key(a, o))
+
+
+def grid_keys(xyz, origin) -> np.ndarray:
+    """Host evaluation of kldi_grid_key for an [n][3] array of points (no GPU needed)."""
+    a = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
+    o = (C.c_double * 3)(*[float(v) for v in origin])
+    out = np.empty(a.shape[0], dtype=np.uint64)
+    _check(lib().kldi_grid_keys(C.c_void_p(a.ctypes.data), a.shape[0], o, C.c_void_p(out.ctypes.data)), "kldi_grid_keys")
+    return out
 
 
 def vsched(nb: int, square: bool = False):

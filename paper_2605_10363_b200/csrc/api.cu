@@ -3,6 +3,8 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 
 #include "kldi_internal.h"
@@ -15,6 +17,17 @@ void set_error(const char* fmt, ...) {
   va_start(ap, fmt);
   vsnprintf(g_err, sizeof(g_err), fmt, ap);
   va_end(ap);
+}
+
+kldi_status ensure_smem_attr(const void* func, int bytes, int device) {
+  static std::mutex mu;
+  static std::map<const void*, uint64_t> done;  // kernel -> bitmask of devices that have the attribute
+  std::lock_guard<std::mutex> lock(mu);
+  uint64_t& m = done[func];
+  if (device >= 0 && device < 64 && ((m >> device) & 1)) return KLDI_OK;
+  KLDI_CUDA(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  if (device >= 0 && device < 64) m |= 1ull << device;
+  return KLDI_OK;
 }
 
 // ------------------------------------------------------------------ FP64 pipe microbenchmark
@@ -83,6 +96,16 @@ uint64_t kldi_grid_key(const double* xyz, const double* origin) {
   return grid_key_host(xyz[0], xyz[1], xyz[2], origin[0], origin[1], origin[2]);
 }
 
+kldi_status kldi_grid_keys(const double* xyz, int64_t n, const double* origin, uint64_t* keys) {
+  if (!xyz || !origin || !keys || n < 0) {
+    set_error("kldi_grid_keys: null argument");
+    return KLDI_EINVAL;
+  }
+  for (int64_t i = 0; i < n; ++i)
+    keys[i] = grid_key_host(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], origin[0], origin[1], origin[2]);
+  return KLDI_OK;
+}
+
 kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid, double eps,
                              int want_gradients, void* cuda_stream, kldi_plan** out) {
   if (out) *out = nullptr;
@@ -104,7 +127,7 @@ kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells,
   P->eps = eps;
   P->want_grad = want_gradients ? 1 : 0;
   cudaGetDevice(&P->device);
-  cudaDeviceProp prop;
+  cudaDeviceProp prop{};
   if (cudaGetDeviceProperties(&prop, P->device) != cudaSuccess || prop.major < 10) {
     set_error("kldi_plan_create: device is not sm_100+ (found sm_%d%d)", prop.major, prop.minor);
     delete P;
@@ -151,6 +174,7 @@ kldi_status kldi_plan_create(const kldi_atoms* atoms, const kldi_shells* shells,
 
 kldi_status kldi_plan_destroy(kldi_plan* P) {
   if (!P) return KLDI_OK;
+  DeviceGuard dev_guard(P->device);
   plan_free(P);
   delete P;
   return KLDI_OK;
@@ -161,7 +185,9 @@ kldi_status kldi_plan_stats(const kldi_plan* P, kldi_stats* out) {
     set_error("kldi_plan_stats: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   *out = P->stats;
+  out->kernel_launches = P->launches;
   out->pair_stages_total = out->pair_stages_executed = -1;
   if (P->pair_counts_valid) {  // counters of the most recent rho contraction run with KLDI_OPT_PAIR_TEST
     unsigned long long c[2] = {0, 0};
@@ -180,12 +206,14 @@ kldi_status kldi_eval_rho(kldi_plan* P, const double* D, double* rho, double* dr
     set_error("kldi_eval_rho: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (drho && !P->want_grad) {
     set_error("kldi_eval_rho: gradients requested from a plan created with want_gradients = 0");
     return KLDI_ESTATE;
   }
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   EV(0);
   if ((rc = launch_permute_D(P, D, drho != nullptr)) != KLDI_OK) return rc;
   EV(1);
@@ -202,12 +230,14 @@ kldi_status kldi_build_vxc(kldi_plan* P, const double* wv, int gga, double* V) {
     set_error("kldi_build_vxc: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (gga && !P->want_grad) {
     set_error("kldi_build_vxc: GGA form requested from a plan created with want_gradients = 0");
     return KLDI_ESTATE;
   }
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   for (int i = 0; i < 4; ++i) EV(i);
   if ((rc = launch_gather_wv(P, wv, gga != 0)) != KLDI_OK) return rc;
   EV(4);
@@ -223,6 +253,7 @@ static kldi_status exc_enqueue(kldi_plan* P, const double* D, kldi_functional f,
   const bool gga = (f == KLDI_GGA_PBEX);
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   EV(0);
   if ((rc = launch_permute_D(P, D, gga)) != KLDI_OK) return rc;
   EV(1);
@@ -249,6 +280,7 @@ kldi_status kldi_exc(kldi_plan* P, const double* D, kldi_functional f, double* E
     set_error("kldi_exc: null argument or unknown functional");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (f == KLDI_GGA_PBEX && !P->want_grad) {
     set_error("kldi_exc: GGA functional needs a plan created with want_gradients = 1");
     return KLDI_ESTATE;
@@ -265,6 +297,7 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
     set_error("kldi_exc_host: null argument or unknown functional");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (f == KLDI_GGA_PBEX && !P->want_grad) {
     set_error("kldi_exc_host: GGA functional needs a plan created with want_gradients = 1");
     return KLDI_ESTATE;
@@ -287,7 +320,18 @@ kldi_status kldi_exc_host(kldi_plan* P, const double* D_host, kldi_functional f,
   }
   kldi_status rc = exc_enqueue(P, dD, f, dV);
   if (rc != KLDI_OK) return rc;
-  if (V_host) KLDI_CUDA(cudaMemcpyAsync(V_host, dV, nn, cudaMemcpyDeviceToHost, P->stream));
+  if (V_host && P->host_v_triangle) {
+    // V is exactly symmetric: download the lower triangle only, in the same 32 row bands as the upload of D
+    const int n = P->n_ao, nb = n < 1024 ? 1 : 32;
+    for (int b = 0; b < nb; ++b) {
+      const int r0 = (int)((int64_t)n * b / nb), r1 = (int)((int64_t)n * (b + 1) / nb);
+      if (r1 > r0)
+        KLDI_CUDA(cudaMemcpy2DAsync(V_host + (size_t)r0 * n, sizeof(double) * n, dV + (size_t)r0 * n, sizeof(double) * n,
+                                    sizeof(double) * r1, r1 - r0, cudaMemcpyDeviceToHost, P->stream));
+    }
+  } else if (V_host) {
+    KLDI_CUDA(cudaMemcpyAsync(V_host, dV, nn, cudaMemcpyDeviceToHost, P->stream));
+  }
   KLDI_CUDA(cudaStreamSynchronize(P->stream));
   *Exc = *P->h_E;
   return KLDI_OK;
@@ -298,12 +342,14 @@ kldi_status kldi_eval_tau(kldi_plan* P, const double* D, double* tau) {
     set_error("kldi_eval_tau: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (!P->want_grad) {
     set_error("kldi_eval_tau: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
     return KLDI_ESTATE;
   }
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   EV(0);
   if ((rc = launch_permute_D(P, D, false)) != KLDI_OK) return rc;  // triangular D': the product is symmetric in mu, nu
   EV(1);
@@ -322,12 +368,14 @@ kldi_status kldi_build_vtau(kldi_plan* P, const double* wv_tau, double* V) {
     set_error("kldi_build_vtau: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (!P->want_grad) {
     set_error("kldi_build_vtau: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
     return KLDI_ESTATE;
   }
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   for (int i = 0; i < 4; ++i) EV(i);
   if ((rc = launch_gather_wv(P, wv_tau, false, 0.5)) != KLDI_OK) return rc;
   EV(4);
@@ -344,6 +392,7 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
     set_error("kldi_exc_grad: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (f != KLDI_LDA_SLATER) {
     set_error("kldi_exc_grad: only KLDI_LDA_SLATER is built (a GGA gradient needs the AO second derivatives)");
     return KLDI_EINVAL;
@@ -355,6 +404,7 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
   if (!P->d_x) KLDI_CUDA(cudaMalloc(&P->d_x, sizeof(double) * GB * (size_t)(P->total_cols + 64)));
   kldi_status rc;
   P->have_timings = false;
+  P->launches = 0;
   EV(0);
   if ((rc = launch_permute_D(P, D, true)) != KLDI_OK) return rc;  // full D: the gradient needs X = Phi D itself
   EV(1);
@@ -375,7 +425,7 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
 
 kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
   if (!P || (option != KLDI_OPT_DETERMINISTIC_V && option != KLDI_OPT_PAIR_TEST && option != KLDI_OPT_RHO_DFMA &&
-             option != KLDI_OPT_RHO_TC)) {
+             option != KLDI_OPT_RHO_TC && option != KLDI_OPT_HOST_V_TRIANGLE)) {
     set_error("kldi_plan_set_option: null plan or unknown option %d", (int)option);
     return KLDI_EINVAL;
   }
@@ -388,6 +438,7 @@ kldi_status kldi_plan_set_option(kldi_plan* P, kldi_option option, int value) {
   }
   if (option == KLDI_OPT_RHO_DFMA) P->rho_impl = value ? 1 : 0;
   if (option == KLDI_OPT_RHO_TC) P->rho_impl = value ? 2 : 0;
+  if (option == KLDI_OPT_HOST_V_TRIANGLE) P->host_v_triangle = value ? 1 : 0;
   if (option == KLDI_OPT_PAIR_TEST) {
     P->pair_test = value ? 1 : 0;
     if (!value) P->pair_counts_valid = false;
@@ -400,6 +451,7 @@ kldi_status kldi_last_timings(kldi_plan* P, double* out) {
     set_error("kldi_last_timings: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   if (!P->have_timings) {
     set_error("kldi_last_timings: no completed call on this plan");
     return KLDI_ESTATE;
@@ -422,6 +474,7 @@ kldi_status kldi_plan_export(const kldi_plan* P, int which, void* buf, int64_t c
     set_error("kldi_plan_export: null argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   const void* hsrc = nullptr;
   const void* dsrc = nullptr;
   int64_t bytes = 0;
@@ -461,6 +514,7 @@ kldi_status kldi_plan_export_tile(const kldi_plan* P, int64_t entry, int c, doub
     set_error("kldi_plan_export_tile: bad argument");
     return KLDI_EINVAL;
   }
+  DeviceGuard dev_guard(P->device);
   // grid block of the entry: binary search in row_ptr
   int64_t lo = 0, hi = P->n_blocks;
   while (hi - lo > 1) {

@@ -656,7 +656,7 @@ kldi_status launch_grad_cols(kldi_plan* P, double* grad) {
   if (P->n_tasks == 0) return KLDI_OK;
   k_grad_cols<<<P->n_tasks, 256, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_colidx, P->d_ao_atom_c,
                                                  P->d_x, P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_wv_s, grad);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
@@ -709,15 +709,12 @@ __global__ void k_finalise_V(const double* __restrict__ Vp, const int32_t* __res
 }
 
 // ===================================================================================== launchers
-static int g_attr_done = 0;
-static kldi_status set_attrs() {
-  if (g_attr_done) return KLDI_OK;
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<false, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES_F));
-  KLDI_CUDA(cudaFuncSetAttribute(k_rho<true, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rho::SMEM_BYTES));
-  g_attr_done = 1;
-  return KLDI_OK;
+static kldi_status set_attrs(const kldi_plan* P) {
+  kldi_status rc;
+  if ((rc = ensure_smem_attr((const void*)k_rho<false, true>, rho::SMEM_BYTES, P->device)) != KLDI_OK) return rc;
+  if ((rc = ensure_smem_attr((const void*)k_rho<true, false>, rho::SMEM_BYTES, P->device)) != KLDI_OK) return rc;
+  if ((rc = ensure_smem_attr((const void*)k_rho<false, true, 1>, rho::SMEM_BYTES_F, P->device)) != KLDI_OK) return rc;
+  return ensure_smem_attr((const void*)k_rho<true, false, 2>, rho::SMEM_BYTES, P->device);
 }
 
 kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
@@ -726,12 +723,12 @@ kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
     k_permute_D<false><<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
   else
     k_permute_D<true><<<grid, 256, 0, P->stream>>>(D, P->d_ao_perm, P->n_ao, P->d_Dp);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
-  kldi_status rc = set_attrs();
+  kldi_status rc = set_attrs(P);
   if (rc != KLDI_OK) return rc;
   if (!gga && P->rho_impl == 2 && !P->pair_test) return launch_rho_tc(P);
   KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
@@ -762,14 +759,14 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
                                                             P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr,
                                                             nullptr, P->d_Dp, P->n_ao, P->d_rho_s, nullptr, P->n_pad,
                                                             pm, nullptr);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 // The LDA-form (triangular D') rho build on another store of the rho layout: out_s[g] = sum_{mu,nu} D_{mu,nu}
 // A_{g,mu} A_{g,nu} with A = d_c Phi (kinetic-energy density).  D' must already be in P->d_Dp.
 kldi_status launch_rho_lda_on(kldi_plan* P, const double* store, double* out_s) {
-  kldi_status rc = set_attrs();
+  kldi_status rc = set_attrs(P);
   if (rc != KLDI_OK) return rc;
   KLDI_CUDA(cudaMemsetAsync(out_s, 0, sizeof(double) * P->n_pad, P->stream));
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
@@ -778,21 +775,21 @@ kldi_status launch_rho_lda_on(kldi_plan* P, const double* store, double* out_s) 
   k_rho<false, true><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, store, nullptr, nullptr, nullptr,
       P->d_Dp, P->n_ao, out_s, nullptr, P->n_pad, nullptr, nullptr);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 kldi_status launch_tau_combine(kldi_plan* P) {
   const int nb = (int)((P->n_pad + 255) / 256);
   k_tau_combine<<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_drho_s, P->d_rho_s);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho) {
   const int nb = (int)((P->n_pad + 255) / 256);
   k_unpermute_rho<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, P->d_rho_s, P->d_drho_s, rho, drho);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
@@ -802,16 +799,16 @@ kldi_status launch_xc(kldi_plan* P, kldi_functional f) {
     k_xc<true><<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_rho_s, P->d_drho_s, P->d_gw, P->d_wv_s, P->d_epart);
   else
     k_xc<false><<<nb, 256, 0, P->stream>>>(P->n_pad, P->d_rho_s, nullptr, P->d_gw, P->d_wv_s, P->d_epart);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   k_sum_partials<<<1, 1024, 0, P->stream>>>(P->d_epart, nb, P->d_E);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 kldi_status launch_gather_wv(kldi_plan* P, const double* wv, bool gga, double scale) {
   const int nb = (int)((P->n_pad + 255) / 256);
   k_gather_wv<<<nb, 256, 0, P->stream>>>(P->d_perm_g, P->n_pad, P->n_pts, gga ? 4 : 1, wv, P->d_wv_s, scale);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
@@ -826,7 +823,7 @@ kldi_status launch_finalise_V(kldi_plan* P, bool gga, double* V, int fixed) {
     k_finalise_V<false, true><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, P->d_fx);
   else
     k_finalise_V<false, false><<<grid, 256, 0, P->stream>>>(P->d_Vp, P->d_ao_perm, P->n_ao, V, nullptr);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 

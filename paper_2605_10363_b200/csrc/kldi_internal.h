@@ -27,7 +27,8 @@ __host__ __device__ __forceinline__ int64_t vlayout_off(int64_t panel_off_p, int
 // Fixed-point scale of the V accumulation: the power of two that maps |x| <= bound below 2^61.
 __host__ __device__ __forceinline__ double fx_scale(double bound) {
   if (!(bound > 0.0)) return 1.0;
-  return scalbn(1.0, 60 - ilogb(bound));
+  const int e = 60 - ilogb(bound);
+  return scalbn(1.0, e > 1000 ? 1000 : e);  // a denormal-small bound would overflow the scale
 }
 
 #define KLDI_CUDA(call)                                                                     \
@@ -37,6 +38,29 @@ __host__ __device__ __forceinline__ double fx_scale(double bound) {
       kldi::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
       return e__ == cudaErrorMemoryAllocation ? KLDI_ENOMEM : KLDI_ECUDA;                   \
     }                                                                                       \
+  } while (0)
+
+// The > 48 KB dynamic-shared-memory opt-in belongs to the device's context: remember per (kernel, device), thread-safe.
+kldi_status ensure_smem_attr(const void* func, int bytes, int device);
+
+// A plan is bound to the device that was current at kldi_plan_create; every entry point runs with that device
+// current and restores the caller's on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
+// after a kernel launch on plan P: check the launch and count it (kldi_stats.kernel_launches)
+#define KLDI_LAUNCHED(P)               \
+  do {                                 \
+    KLDI_CUDA(cudaGetLastError());     \
+    ++(P)->launches;                   \
   } while (0)
 
 // Device-side view of the basis in the plan's spatial shell order.
@@ -106,7 +130,7 @@ struct kldi_plan {
   double* d_tau = nullptr;                        // [2][n_ao] column scales of D', column maxima
   int64_t* d_chunk_off = nullptr;                 // [n_blocks+1] first 32-column chunk of grid block p
   int64_t tc_chunks = 0;
-  int v_mode = 0;                                 // 0: red.global.add.f64 epilogue, 1: workspace + fixed-order reduce,
+  int v_mode = 2;                                 // 0: red.global.add.f64 epilogue, 1: workspace + fixed-order reduce,
                                                   // 2: 64-bit fixed-point integer atomics (reproducible)
   double* d_fx = nullptr;                         // [1 + n_blocks] fixed-point bound, then s_p = sum_g |wv_g| per block
   // ---- executable-pair selection (pairsel.cu), allocated on first use
@@ -129,6 +153,8 @@ struct kldi_plan {
   double* h_E = nullptr;           // pinned
   cudaEvent_t ev[8] = {};
   bool have_timings = false;
+  int64_t launches = 0;            // kernels launched by the current / most recent compute call
+  int host_v_triangle = 0;         // KLDI_OPT_HOST_V_TRIANGLE
 
   // ---- host copies kept for export / tests
   std::vector<int32_t> h_row_ptr, h_col_idx, h_blk_col0, h_col_ptr, h_row_idx, h_pos, h_shell_perm, h_ao_perm;

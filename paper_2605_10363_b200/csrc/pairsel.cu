@@ -88,11 +88,11 @@ kldi_status launch_pair_select(kldi_plan* P, bool tri) {
   if (P->n_tasks == 0) return KLDI_OK;
   dim3 g((P->n_shells + 127) / 128, P->n_shells);
   k_dmax<<<g, 128, 0, P->stream>>>(P->d_Dp, P->n_ao, P->n_shells, P->d_sh_ao0, tri ? 1 : 0, P->d_bmax);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   k_pair_select<<<(P->n_tasks + 3) / 4, 128, 0, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_sh_ao0, P->d_blk_amax, P->d_kp,
       P->d_bmax, P->n_shells, P->eps, tri ? 1 : 0, P->d_pmask, P->d_pcount);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   P->pair_counts_valid = true;
   return KLDI_OK;
 }

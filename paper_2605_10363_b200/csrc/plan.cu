@@ -1,6 +1,7 @@
 // Plan stage of libkldi: once per geometry.
-//   P1 grid reorder      — 60-bit Morton keys (Eq. 20), stable radix sort, blocks of 128
-//   P2 AO partition      — atoms in Morton order, one AO block per shell
+//   P1 grid reorder      — 60-bit space-filling-curve keys on Eq. 20's lattice (the Hilbert index,
+//                          hilbert_key below; Eq. 20's own Z-order key is kept as morton_key), stable radix sort, blocks of 128
+//   P2 AO partition      — atoms in the same curve order, one AO block per shell
 //   P3 AO evaluation     — Cartesian Gaussian shells on (grid block, shell) tiles (Eq. 2)
 //   P4 block filter      — a_pq = max|Phi_pq|, keep iff a_pq >= eps (Eq. 11-13)
 //   P5 BCS build         — BCS(R) row_ptr/col_idx/data and BCS(C) col_ptr/row_idx/pos
@@ -418,7 +419,10 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   kldi_status rc;
   int32_t* d_atom_sh0 = nullptr;
 #define UP(dst, vec)                                    \
-  if ((rc = upload(&(dst), (vec), st)) != KLDI_OK) return rc
+  if ((rc = upload(&(dst), (vec), st)) != KLDI_OK) {    \
+    cudaFree(d_atom_sh0); /* the only temporary so far; the plan's own buffers go in plan_free */ \
+    return rc;                                          \
+  }
   UP(P->d_atom_xyz, h_axyz);
   UP(P->d_sh_atom, h_sh_atom);
   UP(P->d_sh_l, h_sh_l);
@@ -619,7 +623,10 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   constexpr int TASK_BUCKET = 96;
   std::stable_sort(h_tasks.begin(), h_tasks.end(),
                    [&](int32_t a, int32_t b) { return h_kp[a] / TASK_BUCKET > h_kp[b] / TASK_BUCKET; });
-  UP(P->d_tasks, h_tasks);
+  if ((rc = upload(&P->d_tasks, h_tasks, st)) != KLDI_OK) {
+    cleanup();
+    return rc;
+  }
   P->n_tasks = (int32_t)h_tasks.size();
   {
     const kldi_status rcv = vsched_upload(P, h_kp, h_sh_ao0);

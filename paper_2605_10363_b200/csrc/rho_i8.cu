@@ -503,6 +503,25 @@ static kldi_status tc_prepare(kldi_plan* P) {
     h_chunk[p + 1] = h_chunk[p] + (k8 + tc::KC - 1) / tc::KC;
   }
   P->tc_chunks = h_chunk[P->n_blocks];
+  {  // int8 operations the contraction issues (mirrors the producer / MMA issuer loops of k_rho_i8)
+    double ops = 0.0;
+    const int npair = NSL * (NSL + 1) / 2;
+    for (int64_t p = 0; p < P->n_blocks; ++p) {
+      const int k8 = (int)(P->h_panel_off[p + 1] - P->h_panel_off[p]);
+      if (!k8) continue;
+      const int K32 = (k8 + tc::KC - 1) & ~(tc::KC - 1), ntile = (K32 + tc::NT - 1) / tc::NT;
+      const int W = ((K32 / tc::KC + ntile - 1) / ntile) * tc::KC;
+      for (int jt = 0; jt < ntile; ++jt) {
+        const int n0 = jt * W, Wj = std::min(W, K32 - n0);
+        for (int k0 = K32 - tc::KC; k0 >= n0; k0 -= tc::KC) {
+          const int wact = std::min(Wj, k0 + tc::KC - n0);
+          // full-width chunks pair the D' planes at the tile pitch NT (plane rows beyond Wj are issued too)
+          ops += 2.0 * GB * tc::KC * npair * (wact == Wj ? tc::NT : wact);
+        }
+      }
+    }
+    P->stats.ops_rho_tc = ops;
+  }
   KLDI_CUDA(cudaMalloc(&P->d_chunk_off, sizeof(int64_t) * (P->n_blocks + 1)));
   KLDI_CUDA(cudaMemcpyAsync(P->d_chunk_off, h_chunk.data(), sizeof(int64_t) * (P->n_blocks + 1), cudaMemcpyHostToDevice, P->stream));
   KLDI_CUDA(cudaStreamSynchronize(P->stream));  // h_chunk goes out of scope
@@ -514,9 +533,8 @@ static kldi_status tc_prepare(kldi_plan* P) {
   if (P->n_tasks > 0) {
     tc::k_slice_phi<NSL><<<P->n_tasks, 128, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_phi,
                                                            P->d_sigma, P->d_phiq);
-    KLDI_CUDA(cudaGetLastError());
+    KLDI_LAUNCHED(P);
   }
-  KLDI_CUDA(cudaFuncSetAttribute(tc::k_rho_i8<NSL>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NSL>::SMEM_BYTES));
   P->stats.phi_bytes += (int64_t)P->tc_chunks * NSL * tc::A_SLICE;
   return KLDI_OK;
 }
@@ -526,6 +544,7 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   constexpr int NSL = 5;
   kldi_status rc = tc_prepare<NSL>(P);
   if (rc != KLDI_OK) return rc;
+  if ((rc = ensure_smem_attr((const void*)tc::k_rho_i8<NSL>, tc::Cfg<NSL>::SMEM_BYTES, P->device)) != KLDI_OK) return rc;
   KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
   if (P->n_tasks == 0) return KLDI_OK;
@@ -533,9 +552,9 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   double* cmax = P->d_tau + n;
   KLDI_CUDA(cudaMemsetAsync(cmax, 0, sizeof(double) * n, P->stream));
   tc::k_colmax<<<dim3((n + 31) / 32, (n + 255) / 256), 256, 0, P->stream>>>(P->d_Dp, n, reinterpret_cast<unsigned long long*>(cmax));
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   static const bool debug = getenv("KLDI_TC_DEBUG") != nullptr;  // per-role wait cycles, printed to stderr (synchronises)
   long long* dbg = nullptr;
@@ -546,7 +565,7 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phi, P->d_phiq,
       P->d_sigma, P->d_Dq, P->d_tau, n, P->d_rho_s, dbg);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   if (debug) {
     long long h[32];
     KLDI_CUDA(cudaStreamSynchronize(P->stream));

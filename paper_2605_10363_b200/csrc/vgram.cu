@@ -370,19 +370,18 @@ static kldi_status launch_fx_bound(kldi_plan* P, bool gga) {
   KLDI_CUDA(cudaMemsetAsync(P->d_fx, 0, sizeof(double), P->stream));
   k_fx_block_sums<<<(int)((P->n_blocks + 7) / 8), 256, 0, P->stream>>>(P->n_blocks, P->n_pad, gga ? 4 : 1, P->d_wv_s,
                                                                       P->d_fx + 1);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   k_fx_bound<<<P->n_shells, 256, 0, P->stream>>>(P->d_col_ptr, P->d_row_idx, P->d_pos, P->d_blk_amax, P->d_fx + 1,
                                                  P->d_fx);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 template <bool GGA, int EPI>
 static kldi_status launch_vgram(kldi_plan* P, const double* phi_v = nullptr) {
-  static bool attr_done = false;
-  if (!attr_done) {
-    KLDI_CUDA(cudaFuncSetAttribute(k_vgram<GGA, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, vg::SMEM_BYTES));
-    attr_done = true;
+  {
+    const kldi_status rc_attr = ensure_smem_attr((const void*)k_vgram<GGA, EPI>, vg::SMEM_BYTES, P->device);
+    if (rc_attr != KLDI_OK) return rc_attr;
   }
   const int m = GGA ? 1 : 0;
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
@@ -391,7 +390,7 @@ static kldi_status launch_vgram(kldi_plan* P, const double* phi_v = nullptr) {
       P->d_wv_s,
       P->d_vsched_ptr[m], static_cast<const VPass*>(P->d_vpasses[m]), static_cast<const VItem*>(P->d_vitems[m]),
       P->n_ao, P->d_Vp, P->d_gram_off[m], P->d_gram, P->d_fx);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
@@ -488,7 +487,7 @@ static kldi_status launch_vreduce(kldi_plan* P) {
   k_vreduce<GGA><<<(P->n_ao + wpb - 1) / wpb, 32 * wpb, smem, P->stream>>>(
       P->n_ao, P->d_ao_shell, P->d_sh_ao0, P->d_col_ptr, P->d_row_idx, P->d_pos, P->d_blk_col0, P->d_kp,
       P->d_panel_off, P->d_gram_off[m], P->d_colidx, P->d_gram, P->d_Vp);
-  KLDI_CUDA(cudaGetLastError());
+  KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
@@ -502,7 +501,7 @@ kldi_status launch_vxc(kldi_plan* P, bool gga) {
   if (gga) {
     k_build_z<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_kp, P->d_panel_off, P->n_pad, P->d_wv_s, P->d_phi,
                                                        P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_z);
-    KLDI_CUDA(cudaGetLastError());
+    KLDI_LAUNCHED(P);
   }
   if (P->v_mode == 0) return gga ? launch_vgram<true, 0>(P) : launch_vgram<false, 0>(P);
   if (P->v_mode == 2) {
@@ -544,7 +543,7 @@ kldi_status launch_vtau(kldi_plan* P) {
   if (P->v_mode != 0 && (rc = launch_fx_bound(P, false)) != KLDI_OK) return rc;
   for (int c = 0; c < 3; ++c) {
     k_relayout_v<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_panel_off, P->d_dphi[c], P->d_z);
-    KLDI_CUDA(cudaGetLastError());
+    KLDI_LAUNCHED(P);
     KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
     rc = P->v_mode != 0 ? launch_vgram<false, 2>(P, P->d_z) : launch_vgram<false, 0>(P, P->d_z);
     if (rc != KLDI_OK) return rc;
