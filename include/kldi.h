@@ -256,6 +256,22 @@ kldi_status kldi_vsched_export(int nb, int square, int32_t* passes, int32_t* ite
  * column panel_off in the V layout (4 slabs of 32 rows, [col][32] each, 16-byte chunks XOR-swizzled by col & 7). */
 int64_t kldi_vlayout_offset(int64_t panel_off, int32_t K8, int32_t col, int32_t row);
 
+/* Overlap-signature ordering of the AO blocks (Eq. 8-10, Eq. 21),
+ * host only, no GPU needed: the overlap matrix S in closed form, signatures = rows of the atom-block norms
+ * T_AB = ||S_AB||_F (the clustered unit is the centre: its shells are the AO blocks and stay together), cosine distance
+ * d(A,B) = 1 - s_A.s_B/(|s_A||s_B|), agglomerative clustering with average linkage, the two sub-trees of every merge
+ * oriented so that the closest of their end leaves become adjacent; order[r] = caller atom at position r.  mode must be
+ * 1.  dist: HOST [n_atoms][n_atoms] cosine distances or NULL.  At most 4096 centres (KLDI_EINVAL beyond). */
+kldi_status kldi_ao_order(const kldi_atoms* atoms, const kldi_shells* shells, int mode, int32_t* order, double* dist);
+
+/* Process-wide defaults of plans created afterwards.  KLDI_DEFAULT_AO_ORDER: order of the atoms (and so of the AO
+ * blocks) inside the plan: 0 (default) = along the same space-filling curve as the grid; 1 = kldi_ao_order's
+ * overlap-signature clustering (falls back to 0 beyond 4096 centres); 2 = the caller's order.  The order is internal:
+ * results do not depend on it (tested); with per-shell filtering and packed panels it does not change K_p either, only
+ * the locality of the D gather and of the V scatter. */
+typedef enum { KLDI_DEFAULT_AO_ORDER = 1 } kldi_plan_default;
+kldi_status kldi_set_plan_default(kldi_plan_default what, int value);
+
 const char* kldi_last_error(void);
 
 #ifdef __cplusplus

@@ -22,7 +22,7 @@ EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_exc_grad", "kldi_eval_tau", "kldi_build_vtau", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
     "kldi_morton_key", "kldi_grid_key", "kldi_grid_keys", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
-    "kldi_vlayout_offset",
+    "kldi_vlayout_offset", "kldi_ao_order", "kldi_set_plan_default",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
 KLDI_OPT_PAIR_TEST = 2
@@ -99,6 +99,8 @@ def lib():
         L.kldi_grid_key.restype = C.c_uint64
         L.kldi_grid_keys.argtypes = [C.c_void_p, C.c_int64, C.POINTER(C.c_double), C.c_void_p]
         L.kldi_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.kldi_ao_order.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.kldi_set_plan_default.argtypes = [C.c_int, C.c_int]
         L.kldi_vsched_export.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_vlayout_offset.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         L.kldi_vlayout_offset.restype = C.c_int64
@@ -300,6 +302,29 @@ def grid_key(xyz, origin) -> int:
     a = (C.c_double * 3)(*[float(v) for v in xyz])
     o = (C.c_double * 3)(*[float(v) for v in origin])
     return int(lib().kldi_grid_key(a, o))
+
+
+KLDI_DEFAULT_AO_ORDER = 1
+AO_ORDER_CURVE, AO_ORDER_OVERLAP, AO_ORDER_CALLER = 0, 1, 2
+
+
+def set_plan_default(what: int, value: int) -> None:
+    """Process-wide default of plans created afterwards (kldi_set_plan_default)."""
+    _check(lib().kldi_set_plan_default(int(what), int(value)), "kldi_set_plan_default")
+
+
+def ao_order(atom_xyz, shell_atom, shell_l, shell_prim_off, prim_alpha, prim_coef, want_dist: bool = False):
+    """Host-only: overlap-signature order of the atoms (kldi_ao_order) -> order[, cosine distance matrix]."""
+    ax = _np(atom_xyz, np.float64)
+    sa, sl, so = _np(shell_atom, np.int32), _np(shell_l, np.int32), _np(shell_prim_off, np.int32)
+    pa, pc = _np(prim_alpha, np.float64), _np(prim_coef, np.float64)
+    atoms = _Atoms(ax.shape[0], ax.ctypes.data)
+    shells = _Shells(sa.shape[0], sa.ctypes.data, sl.ctypes.data, so.ctypes.data, pa.ctypes.data, pc.ctypes.data)
+    order = np.empty(ax.shape[0], dtype=np.int32)
+    dist = np.empty((ax.shape[0], ax.shape[0])) if want_dist else None
+    _check(lib().kldi_ao_order(C.byref(atoms), C.byref(shells), 1, C.c_void_p(order.ctypes.data),
+                               C.c_void_p(dist.ctypes.data) if want_dist else None), "kldi_ao_order")
+    return (order, dist) if want_dist else order
 
 
 def grid_keys(xyz, origin) -> np.ndarray:

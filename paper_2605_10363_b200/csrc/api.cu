@@ -80,9 +80,43 @@ __global__ void __launch_bounds__(256) k_peak_mix(int iters, double* sink) {
 }
 }  // namespace kldi
 
+namespace kldi {
+int g_default_ao_order = 0;
+}
+
 using namespace kldi;
 
 extern "C" {
+
+kldi_status kldi_set_plan_default(kldi_plan_default what, int value) {
+  if (what != KLDI_DEFAULT_AO_ORDER || value < 0 || value > 2) {
+    set_error("kldi_set_plan_default: unknown default %d or value %d", (int)what, value);
+    return KLDI_EINVAL;
+  }
+  g_default_ao_order = value;
+  return KLDI_OK;
+}
+
+kldi_status kldi_ao_order(const kldi_atoms* atoms, const kldi_shells* shells, int mode, int32_t* order, double* dist) {
+  if (!atoms || !shells || !order || atoms->n_atoms <= 0 || mode != 1) {
+    set_error("kldi_ao_order: null argument or unsupported mode");
+    return KLDI_EINVAL;
+  }
+  for (int s = 0; s < shells->n_shells; ++s)
+    if (shells->l[s] < 0 || shells->l[s] > 2 || shells->atom[s] < 0 || shells->atom[s] >= atoms->n_atoms) {
+      set_error("kldi_ao_order: shell %d not supported", s);
+      return KLDI_EINVAL;
+    }
+  std::vector<int> o;
+  std::vector<double> d;
+  if (!overlap_signature_order(atoms, shells, o, dist ? &d : nullptr)) {
+    set_error("kldi_ao_order: more than 4096 centres");
+    return KLDI_EINVAL;
+  }
+  for (int a = 0; a < atoms->n_atoms; ++a) order[a] = o[a];
+  if (dist) std::copy(d.begin(), d.end(), dist);
+  return KLDI_OK;
+}
 
 const char* kldi_last_error(void) { return g_err; }
 

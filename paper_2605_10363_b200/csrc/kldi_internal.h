@@ -167,6 +167,10 @@ uint64_t morton_key_host(double x, double y, double z, double x0, double y0, dou
 uint64_t grid_key_host(double x, double y, double z, double x0, double y0, double z0);
 kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells* shells, const kldi_grid* grid);
 void plan_free(kldi_plan* P);
+// aoorder.cu: atom order by overlap-signature clustering; dist_out: the cosine distances
+bool overlap_signature_order(const kldi_atoms* atoms, const kldi_shells* shells, std::vector<int>& order,
+                             std::vector<double>* dist_out = nullptr);
+extern int g_default_ao_order;  // kldi_set_plan_default(KLDI_DEFAULT_AO_ORDER): 0 curve, 1 overlap signature, 2 caller
 // contract.cu
 kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
 // pairsel.cu

@@ -365,6 +365,12 @@ kldi_status plan_build(kldi_plan* P, const kldi_atoms* atoms, const kldi_shells*
   for (int a = 0; a < n_atoms; ++a)
     akey[a] = hilbert_key(atoms->xyz[3 * a], atoms->xyz[3 * a + 1], atoms->xyz[3 * a + 2], a0[0], a0[1], a0[2]);
   std::stable_sort(atom_order.begin(), atom_order.end(), [&](int i, int j) { return akey[i] < akey[j]; });
+  if (g_default_ao_order == 2) {
+    std::iota(atom_order.begin(), atom_order.end(), 0);  // the caller's order (measurement only)
+  } else if (g_default_ao_order == 1) {
+    std::vector<int> o;  // overlap-signature clustering; beyond its size limit the curve order stays
+    if (overlap_signature_order(atoms, shells, o)) atom_order = o;
+  }
   std::vector<int> atom_rank(n_atoms);
   for (int r = 0; r < n_atoms; ++r) atom_rank[atom_order[r]] = r;
 

@@ -721,3 +721,27 @@ def test_exc_host_lower_triangle_download(K):
         untouched[r0:r1, :r1] = False
     assert bool((Vtri[untouched] == 7.0).all()) and int(untouched.sum()) > 0.4 * n * n
     plan.close()
+
+
+def test_ao_order_is_internal(K):
+    """KLDI_DEFAULT_AO_ORDER: curve order, overlap-signature clustering or the
+    caller's order of the atoms inside the plan — the retained set (sum K_p) and the results do not depend on it."""
+    import torch
+
+    wl = W.named_config("cfg1", n_override=10)
+    D = torch.as_tensor(wl.D, device="cuda")
+    ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "lda")
+    sums, perms = [], []
+    try:
+        for mode in (K.AO_ORDER_CURVE, K.AO_ORDER_OVERLAP, K.AO_ORDER_CALLER):
+            K.set_plan_default(K.KLDI_DEFAULT_AO_ORDER, mode)
+            plan = K.Plan.from_workload(wl)
+            E, V = plan.exc(D)
+            check({"rho": plan.eval_rho(D).cpu().numpy(), "V": V.cpu().numpy(), "E": E, "drho": None}, ref)
+            sums.append((int(plan.stats.sum_k), int(plan.stats.retained_blocks)))
+            perms.append(plan.export("ao_perm").copy())
+            plan.close()
+    finally:
+        K.set_plan_default(K.KLDI_DEFAULT_AO_ORDER, K.AO_ORDER_CURVE)
+    assert sums[0] == sums[1] == sums[2]
+    assert not np.array_equal(perms[0], perms[1]) and np.array_equal(perms[2][:15], np.arange(15))
