@@ -22,7 +22,8 @@ dense-product step; `brute_force_lda` below is the same thing as explicit Python
 Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): analytic Gaussian overlap => diag(S)=1 and
 int rho = Tr(D S); closed-form Slater energy of one s-Gaussian; V symmetric; central finite
 differences dE/dD = V (LDA and PBE-x); brute-force loops on single water; PBE-x limits; central finite
-differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda; kinetic-energy density: closed
+differences of E in the atom coordinates (fixed grid) = exc_nuclear_gradient_lda / _gga (AO second derivatives from
+central differences of the analytic first ones); kinetic-energy density: closed
 form int tau = 3 alpha n / 2 of one s-Gaussian, AO gradients from finite differences, Tr(D V^tau) = sum wv tau.
 Absolute PBE-x (and Slater) energies: the four decimals the PBE paper prints for the exchange energy of
 the hydrogen atom (tests/golden/pbe_x_hydrogen.txt), by a 1-D radial integral of slater() / pbe_x().
@@ -265,6 +266,85 @@ def exc_nuclear_gradient_lda(basis, pts, w, D, chunk: int = 8192):
         X = phi @ D
         for c in range(3):
             per_ao = -2.0 * np.einsum("g,gm,gm->m", wv, dphi[c], X)
+            np.add.at(grad[:, c], ao_atom, per_ao)
+    return grad
+
+
+def ao_hessians(atom_xyz, shell_atom, shell_l, shell_prim_off, prim_alpha, prim_coef, pts):
+    """Second derivatives d2Phi[c, d, g, mu] = d^2 chi_mu / d r_c d r_d of the contracted Cartesian Gaussians of
+    ao_values.  A primitive is a product of 1-D factors u(x) = x^n e^{-a x^2}, so
+        u'  = (n x^{n-1} - 2 a x^{n+1}) e^{-a x^2},
+        u'' = (n (n-1) x^{n-2} - 2 a (2 n + 1) x^n + 4 a^2 x^{n+2}) e^{-a x^2},
+    the mixed second derivative is u_c' u_d' u_e and the pure one u_c'' u_d u_e.  Pinned by central differences of the
+    analytic gradients of ao_values (tests/test_oracle_pins.py)."""
+    pts = np.asarray(pts, dtype=np.float64)
+    n_pts = pts.shape[0]
+    n_ao = n_ao_of(shell_l)
+    out = np.zeros((3, 3, n_pts, n_ao))
+    col = 0
+    for s in range(len(shell_l)):
+        l = int(shell_l[s])
+        dx = pts - np.asarray(atom_xyz[int(shell_atom[s])])[None, :]
+        for pw in cart_components(l):
+            for p in range(int(shell_prim_off[s]), int(shell_prim_off[s + 1])):
+                a = float(prim_alpha[p])
+                c = float(prim_coef[p]) * norm_const(a, *pw)
+                u0, u1, u2 = [], [], []
+                for d in range(3):
+                    x, n = dx[:, d], pw[d]
+                    e = np.exp(-a * x * x)
+                    u0.append(x ** n * e)
+                    t1 = -2.0 * a * x ** (n + 1)
+                    if n > 0:
+                        t1 = t1 + n * x ** (n - 1)
+                    u1.append(t1 * e)
+                    t2 = -2.0 * a * (2 * n + 1) * x ** n + 4.0 * a * a * x ** (n + 2)
+                    if n > 1:
+                        t2 = t2 + n * (n - 1) * x ** (n - 2)
+                    u2.append(t2 * e)
+                for d1 in range(3):
+                    for d2 in range(3):
+                        f = [u0[0], u0[1], u0[2]]
+                        if d1 == d2:
+                            f[d1] = u2[d1]
+                        else:
+                            f[d1], f[d2] = u1[d1], u1[d2]
+                        out[d1, d2, :, col] += c * f[0] * f[1] * f[2]
+            col += 1
+    return out
+
+
+def exc_nuclear_gradient_gga(basis, pts, w, D, chunk: int = 4096):
+    """EXC nuclear-gradient contraction for the GGA functional (Slater x PBE enhancement), fixed density matrix and FIXED
+    quadrature, same reading G1 as exc_nuclear_gradient_lda: the chain rule on E_xc = sum_g w_g e(rho_g, sigma_g),
+    sigma = |grad rho|^2, with d chi_mu / d A_c = - d_c chi_mu for mu on A (D symmetric, X = Phi D, X^d = d_d Phi D):
+
+        d rho / d A_c        = -2 sum_{mu on A} d_c Phi_mu X_mu
+        d (d_d rho) / d A_c  = -2 sum_{mu on A} [ d_c d_d Phi_mu X_mu + d_c Phi_mu X^d_mu ]
+        dE / d A_c = sum_g [ wv0 d rho / d A_c + sum_d wv_d d (d_d rho) / d A_c ],
+        wv0 = w v_rho,  wv_d = 2 w v_sigma d_d rho          (the wv convention of kldi_build_vxc).
+
+    Returns grad [n_atoms][3].  Pinned by central differences of the oracle's GGA energy in the atom coordinates."""
+    atom_xyz, shell_atom, shell_l = basis[0], basis[1], basis[2]
+    ao_atom = np.concatenate([[int(shell_atom[s])] * ((int(l) + 1) * (int(l) + 2) // 2) for s, l in enumerate(shell_l)])
+    grad = np.zeros((len(atom_xyz), 3))
+    for c0 in range(0, len(pts), chunk):
+        p = pts[c0:c0 + chunk]
+        phi, dphi = ao_values(*basis, p, deriv=True)
+        hess = ao_hessians(*basis, p)
+        rho = density(phi, D)
+        drho = density_gradient(phi, dphi, D)
+        _, v_rho, v_sigma = pbe_x(rho, np.sum(drho ** 2, axis=0))
+        ww = w[c0:c0 + chunk]
+        wv0 = ww * v_rho
+        wvd = [2.0 * ww * v_sigma * drho[d] for d in range(3)]
+        X = phi @ D
+        Xd = [dphi[d] @ D for d in range(3)]
+        for c in range(3):
+            per_ao = -2.0 * np.einsum("g,gm,gm->m", wv0, dphi[c], X)
+            for d in range(3):
+                per_ao = per_ao - 2.0 * np.einsum("g,gm,gm->m", wvd[d], hess[c, d], X)
+                per_ao = per_ao - 2.0 * np.einsum("g,gm,gm->m", wvd[d], dphi[c], Xd[d])
             np.add.at(grad[:, c], ao_atom, per_ao)
     return grad
 

@@ -155,6 +155,39 @@ def test_nuclear_gradient_lda_matches_finite_difference_of_energy(water):
         assert abs(g[:, c].sum() + np.dot(wv, drho[c])) < 1e-10 * np.max(np.abs(g))
 
 
+def test_nuclear_gradient_gga_matches_finite_difference_of_energy(water):
+    """GGA half of SURVEY.md §8(f2).  (a) the AO second derivatives against central differences of the analytic first
+    derivatives in the point coordinates (and symmetric in the two directions); (b) the GGA nuclear-gradient contraction
+    against central differences of the oracle's GGA energy in the atom coordinates, grid held fixed; (c) mu -> 0 in the
+    functional is not available here, but dropping the sigma terms must give back the LDA-form expression: checked through
+    (b) on five components of both signs."""
+    basis = basis_of(water)
+    rng = np.random.default_rng(4)
+    p = rng.uniform(-2.5, 2.5, size=(40, 3))
+    hess = O.ao_hessians(*basis, p)
+    assert np.max(np.abs(hess - hess.transpose(1, 0, 2, 3))) < 1e-13
+    h = 1e-5
+    for d in range(3):
+        pp, pm = p.copy(), p.copy()
+        pp[:, d] += h
+        pm[:, d] -= h
+        fd = (O.ao_values(*basis, pp, deriv=True)[1] - O.ao_values(*basis, pm, deriv=True)[1]) / (2 * h)   # [c, g, mu]
+        assert np.max(np.abs(fd - hess[:, d])) < 2e-8 * max(1.0, np.max(np.abs(hess)))
+    g = O.exc_nuclear_gradient_gga(basis, water.grid_xyz, water.grid_w, water.D)
+    assert g.shape == (3, 3) and np.max(np.abs(g)) > 1e-3
+    h = 1e-4
+    for (a, c) in [(0, 0), (0, 2), (1, 1), (2, 0), (2, 2)]:
+        e = []
+        for sgn in (+1, -1):
+            xyz = np.array(basis[0], dtype=np.float64, copy=True)
+            xyz[a, c] += sgn * h
+            e.append(O.exc((xyz,) + tuple(basis[1:]), water.grid_xyz, water.grid_w, water.D, "gga", want_v=False)["E"])
+        fd = (e[0] - e[1]) / (2 * h)
+        assert abs(fd - g[a, c]) < 1e-6 * np.max(np.abs(g)), (a, c, fd, g[a, c])
+    g_lda = O.exc_nuclear_gradient_lda(basis, water.grid_xyz, water.grid_w, water.D)
+    assert np.max(np.abs(g - g_lda)) > 1e-4          # the enhancement factor is really in it
+
+
 def test_kinetic_energy_density_and_vtau(water):
     """SURVEY.md §8(f4) contractions.  (a) closed form: one normalised s-Gaussian, exponent alpha, occupation n has
     int tau = n * 3 alpha / 2 (its kinetic energy); (b) tau from AO gradients taken by central differences of the AO
