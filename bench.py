@@ -394,6 +394,12 @@ def main():
                     "grad_contraction_gbs": col_bytes / (tg["vxc"] * 1e-3) / 1e9,
                     "grad_contraction_frac_of_hbm": col_bytes / (tg["vxc"] * 1e-3) / 1e9 / peaks().get("hbm_gbs", 6650.0),
                     "sum_k": sg["sum_k"], "plan_create_s": sg["plan_seconds"]}
+        tgg = []
+        for i in range(3 + min(args.steps, 10)):
+            plan_g.exc_grad(D, K.KLDI_GGA_PBEX)
+            if i >= 3:
+                tgg.append(plan_g.last_timings()["total"])
+        grad_leg["gga_pbex_ms_per_call"] = float(np.median(tgg))
         # the meta-GGA contractions on the same plan (three LDA-form builds each)
         wv_t = torch.as_tensor(wl.grid_w, device="cuda").clone()
         Vt = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")

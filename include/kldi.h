@@ -183,14 +183,16 @@ kldi_status kldi_eval_tau(kldi_plan* plan, const double* D, double* tau);
 kldi_status kldi_build_vtau(kldi_plan* plan, const double* wv_tau, double* V);
 
 /* EXC nuclear-gradient contraction (the paper's second workload; it prints no formula, so this is
- * the chain rule on E_xc = sum_g w_g e(rho_g), DESIGN.md §3 reading G1): at fixed D and FIXED quadrature (points and
- * weights do not follow the atoms, no grid response),
- *     grad[A][c] = dE_xc/dA_c = -2 sum_g w_g v_rho(rho_g) sum_{mu on A} d_c Phi_{g,mu} X_{g,mu},   X = Phi D,
- * over the retained (grid-block, AO-shell) pairs.  LDA only (f = KLDI_LDA_SLATER; anything else -> KLDI_EINVAL); the
- * plan must hold the gradient stores (want_gradients = 1, else KLDI_ESTATE).  D: DEVICE [n_ao][n_ao] row-major,
- * symmetric.  grad: DEVICE [n_atoms][3], caller atom order, overwritten.  Exc: HOST, may be NULL.  The first call
- * allocates an X store of the size of one Phi store, owned by the plan.  Synchronises before it returns.
- * kldi_last_timings: rho = the X / rho build, vxc = the gradient contraction. */
+ * the chain rule on E_xc = sum_g w_g e(rho_g, |grad rho_g|^2), DESIGN.md §3 reading G1): at fixed D and FIXED quadrature
+ * (points and weights do not follow the atoms, no grid response), with X = Phi D and X^d = d_d Phi D,
+ *   KLDI_LDA_SLATER: grad[A][c] = -2 sum_g w_g v_rho sum_{mu on A} d_c Phi_{g,mu} X_{g,mu}
+ *   KLDI_GGA_PBEX  : grad[A][c] = -2 sum_g sum_{mu on A} { wv0 d_c Phi X + sum_d wv_d [ d_c d_d Phi X + d_c Phi X^d ] },
+ *                    wv0 = w v_rho, wv_d = 2 w v_sigma d_d rho (AO second derivatives are evaluated on the fly)
+ * over the retained (grid-block, AO-shell) pairs.  Other functionals -> KLDI_EINVAL; the plan must hold the gradient
+ * stores (want_gradients = 1, else KLDI_ESTATE).  D: DEVICE [n_ao][n_ao] row-major, symmetric.  grad: DEVICE
+ * [n_atoms][3], caller atom order, overwritten.  Exc: HOST, may be NULL.  The first call allocates an X store of the size
+ * of one Phi store (GGA: four), owned by the plan.  Synchronises before it returns.
+ * kldi_last_timings: rho = the X / rho builds, vxc = the gradient contraction. */
 kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, double* Exc, double* grad);
 
 /* Options of a plan (kldi_plan_set_option returns KLDI_EINVAL for an unknown option).

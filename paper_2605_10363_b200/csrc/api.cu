@@ -427,27 +427,36 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
     return KLDI_EINVAL;
   }
   DeviceGuard dev_guard(P->device);
-  if (f != KLDI_LDA_SLATER) {
-    set_error("kldi_exc_grad: only KLDI_LDA_SLATER is built (a GGA gradient needs the AO second derivatives)");
+  if (f != KLDI_LDA_SLATER && f != KLDI_GGA_PBEX) {
+    set_error("kldi_exc_grad: unknown functional");
     return KLDI_EINVAL;
   }
   if (!P->want_grad) {
     set_error("kldi_exc_grad: needs a plan created with want_gradients = 1 (the stores of grad Phi)");
     return KLDI_ESTATE;
   }
-  if (!P->d_x) KLDI_CUDA(cudaMalloc(&P->d_x, sizeof(double) * GB * (size_t)(P->total_cols + 64)));
+  const bool gga = f == KLDI_GGA_PBEX;
+  const size_t store = sizeof(double) * GB * (size_t)(P->total_cols + 64);
+  if (!P->d_x) KLDI_CUDA(cudaMalloc(&P->d_x, store));
+  if (gga && !P->d_xd) KLDI_CUDA(cudaMalloc(&P->d_xd, 3 * store + sizeof(double) * P->n_pad));
   kldi_status rc;
   P->have_timings = false;
   P->launches = 0;
   EV(0);
   if ((rc = launch_permute_D(P, D, true)) != KLDI_OK) return rc;  // full D: the gradient needs X = Phi D itself
   EV(1);
-  if ((rc = launch_rho(P, true, P->d_x)) != KLDI_OK) return rc;
+  // LDA: X-only form (rho + X).  GGA: the GGA form (rho, grad rho and X in one pass), then X^d = d_d Phi D
+  if ((rc = launch_rho(P, true, P->d_x, !gga)) != KLDI_OK) return rc;
+  if (gga) {
+    double* scratch = P->d_xd + 3 * (store / sizeof(double));
+    for (int d = 0; d < 3; ++d)
+      if ((rc = launch_x_on(P, P->d_dphi[d], P->d_xd + d * (store / sizeof(double)), scratch)) != KLDI_OK) return rc;
+  }
   EV(2);
   if ((rc = launch_xc(P, f)) != KLDI_OK) return rc;
   EV(3);
   EV(4);
-  if ((rc = launch_grad_cols(P, grad)) != KLDI_OK) return rc;
+  if ((rc = gga ? launch_grad_cols_gga(P, grad) : launch_grad_cols(P, grad)) != KLDI_OK) return rc;
   EV(5);
   EV(6);
   KLDI_CUDA(cudaMemcpyAsync(P->h_E, P->d_E, sizeof(double), cudaMemcpyDeviceToHost, P->stream));

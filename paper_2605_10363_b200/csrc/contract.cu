@@ -12,6 +12,7 @@
 // FP64 tensor-core MMAs (DMMA.8x8x4) on register accumulators.
 #include <cstdio>
 
+#include "ao_eval.cuh"
 #include "kldi_internal.h"
 #include "ptx.cuh"
 
@@ -543,6 +544,8 @@ __global__ void __launch_bounds__(IMPL == 1 ? 32 * (rho::NCW_F + rho::NPW) : rho
   }
 }
 
+static kldi_status set_attrs(const kldi_plan* P);
+
 // ===================================================================================== H3
 constexpr double C_X = 0.73855876638202240588;    // (3/4)(3/pi)^{1/3}
 constexpr double K_S = 9.5707800006273016908;     // (3 pi^2)^{2/3}
@@ -651,11 +654,93 @@ __global__ void __launch_bounds__(256) k_grad_cols(const int32_t* __restrict__ t
   }
 }
 
+// GGA form (G1):
+//   dE/dA_c = -2 sum_g sum_{mu on A} { wv0 d_c Phi_mu X_mu + sum_d wv_d [ d_c d_d Phi_mu X_mu + d_c Phi_mu X^d_mu ] },
+// wv0 = w v_rho, wv_d = 2 w v_sigma d_d rho (k_xc), X = Phi D and X^d = d_d Phi D from the stores the rho kernel wrote.
+// One CTA per grid block, one thread per grid point; the first and second AO derivatives of a column are evaluated
+// from the shell table (no Hessian store); the columns of a panel ascend in plan AO index, so an atom's columns are
+// consecutive: the three components are summed over them in registers and reduced over the block once per atom.
+__global__ void __launch_bounds__(128) k_grad_cols_gga(ShellTable T, const int32_t* __restrict__ tasks,
+                                                       const int32_t* __restrict__ kp, const int64_t* __restrict__ panel_off,
+                                                       const int32_t* __restrict__ colidx, const int32_t* __restrict__ ao_shell,
+                                                       const int32_t* __restrict__ ao_atom_c, const double* __restrict__ gx,
+                                                       const double* __restrict__ gy, const double* __restrict__ gz,
+                                                       const double* __restrict__ x, const double* __restrict__ xd,
+                                                       int64_t xd_stride, const double* __restrict__ wv_s, int64_t n_pad,
+                                                       double* __restrict__ grad) {
+  __shared__ double red[4][3];
+  const int p = tasks[blockIdx.x], t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int K = kp[p];
+  const int64_t base = panel_off[p], g = (int64_t)p * GB + t;
+  const double px = gx[g], py = gy[g], pz = gz[g];
+  const double w0 = wv_s[g], w1 = wv_s[n_pad + g], w2 = wv_s[2 * n_pad + g], w3 = wv_s[3 * n_pad + g];
+  double acc[3] = {0.0, 0.0, 0.0};
+  int cur_atom = -1;
+  auto flush = [&](int atom) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      double v = acc[c];
+#pragma unroll
+      for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+      if (lane == 0) red[warp][c] = v;
+      acc[c] = 0.0;
+    }
+    __syncthreads();
+    if (t < 3) atomicAdd(grad + 3 * atom + t, -2.0 * (red[0][t] + red[1][t] + red[2][t] + red[3][t]));
+    __syncthreads();
+  };
+  for (int k = 0; k < K; ++k) {
+    const int ao = colidx[base + k];
+    const int atom = ao_atom_c[ao];
+    if (atom != cur_atom) {
+      if (cur_atom >= 0) flush(cur_atom);
+      cur_atom = atom;
+    }
+    const int s = ao_shell[ao];
+    double gr[3], h[6];
+    eval_component_hess(T, s, ao - T.sh_ao0[s], px, py, pz, gr, h);
+    const int64_t o = (base + k) * GB + t;
+    const double X = x[o], X0 = xd[o], X1 = xd[xd_stride + o], X2 = xd[2 * xd_stride + o];
+    const double xw = w0 * X + w1 * X0 + w2 * X1 + w3 * X2;  // multiplies d_c Phi
+    acc[0] += gr[0] * xw + X * (w1 * h[0] + w2 * h[1] + w3 * h[2]);
+    acc[1] += gr[1] * xw + X * (w1 * h[1] + w2 * h[3] + w3 * h[4]);
+    acc[2] += gr[2] * xw + X * (w1 * h[2] + w2 * h[4] + w3 * h[5]);
+  }
+  if (cur_atom >= 0) flush(cur_atom);
+}
+
 kldi_status launch_grad_cols(kldi_plan* P, double* grad) {
   KLDI_CUDA(cudaMemsetAsync(grad, 0, sizeof(double) * 3 * P->n_atoms, P->stream));
   if (P->n_tasks == 0) return KLDI_OK;
   k_grad_cols<<<P->n_tasks, 256, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_colidx, P->d_ao_atom_c,
                                                  P->d_x, P->d_dphi[0], P->d_dphi[1], P->d_dphi[2], P->d_wv_s, grad);
+  KLDI_LAUNCHED(P);
+  return KLDI_OK;
+}
+
+kldi_status launch_grad_cols_gga(kldi_plan* P, double* grad) {
+  KLDI_CUDA(cudaMemsetAsync(grad, 0, sizeof(double) * 3 * P->n_atoms, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  ShellTable T{P->d_atom_xyz, P->d_sh_atom, P->d_sh_l, P->d_sh_prim0, P->d_sh_ao0, P->d_prim_alpha, P->d_prim_cn};
+  const int64_t stride = (int64_t)GB * (P->total_cols + 64);
+  k_grad_cols_gga<<<P->n_tasks, 128, 0, P->stream>>>(T, P->d_tasks, P->d_kp, P->d_panel_off, P->d_colidx, P->d_ao_shell,
+                                                     P->d_ao_atom_c, P->d_gx, P->d_gy, P->d_gz, P->d_x, P->d_xd, stride,
+                                                     P->d_wv_s, P->n_pad, grad);
+  KLDI_LAUNCHED(P);
+  return KLDI_OK;
+}
+
+// X_out = A D for another store A of the rho layout (A = d_d Phi: the X^d of the GGA nuclear gradient), with the X-only
+// form of k_rho; its row sums go to a scratch vector.  The full D must already be in P->d_Dp.
+kldi_status launch_x_on(kldi_plan* P, const double* store, double* x_out, double* rho_scratch) {
+  kldi_status rc = set_attrs(P);
+  if (rc != KLDI_OK) return rc;
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
+  if (P->n_tasks == 0) return KLDI_OK;
+  const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
+  k_rho<true, false, 2><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, store, nullptr, nullptr, nullptr, P->d_Dp,
+      P->n_ao, rho_scratch, nullptr, P->n_pad, nullptr, x_out);
   KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
@@ -727,7 +812,7 @@ kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga) {
   return KLDI_OK;
 }
 
-kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
+kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store, bool x_only) {
   kldi_status rc = set_attrs(P);
   if (rc != KLDI_OK) return rc;
   if (!gga && P->rho_impl == 2 && !P->pair_test) return launch_rho_tc(P);
@@ -741,7 +826,7 @@ kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store) {
     pm = P->d_pmask;
   }
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
-  if (gga && x_store)  // the X build of kldi_exc_grad: rho and the X store, no grad rho
+  if (gga && x_store && x_only)  // the X build of kldi_exc_grad (LDA): rho and the X store, no grad rho
     k_rho<true, false, 2><<<grid, rho::NTHREADS, rho::SMEM_BYTES, P->stream>>>(
         P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_colidx, P->d_phi, nullptr, nullptr, nullptr,
         P->d_Dp, P->n_ao, P->d_rho_s, P->d_drho_s, P->n_pad, pm, x_store);

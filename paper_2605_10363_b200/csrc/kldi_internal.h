@@ -111,6 +111,7 @@ struct kldi_plan {
   double* d_phi_v = nullptr;       // second copy of Phi in the V layout (vlayout_off)
   double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, V layout
   double* d_x = nullptr;           // nuclear gradient: X = Phi D of every panel, rho layout, allocated on first use
+  double* d_xd = nullptr;          // GGA nuclear gradient: X^d = d_d Phi D, d = x, y, z (three stores) + [n_pad] scratch
 
   // ---- V contraction schedule (vsched.h), index 0: LDA upper triangle, 1: GGA square
   int32_t* d_vsched_ptr[2] = {nullptr, nullptr};  // [max_nb + 2] first pass of an nb-block panel
@@ -175,7 +176,9 @@ extern int g_default_ao_order;  // kldi_set_plan_default(KLDI_DEFAULT_AO_ORDER):
 kldi_status launch_permute_D(kldi_plan* P, const double* D, bool gga);
 // pairsel.cu
 kldi_status launch_pair_select(kldi_plan* P, bool tri);
-kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store = nullptr);
+kldi_status launch_rho(kldi_plan* P, bool gga, double* x_store = nullptr, bool x_only = true);
+kldi_status launch_x_on(kldi_plan* P, const double* store, double* x_out, double* rho_scratch);
+kldi_status launch_grad_cols_gga(kldi_plan* P, double* grad);
 // rho_i8.cu
 kldi_status launch_rho_tc(kldi_plan* P);
 kldi_status launch_grad_cols(kldi_plan* P, double* grad);

@@ -325,7 +325,7 @@ void plan_free(kldi_plan* P) {
   if (!P) return;
   cudaSetDevice(P->device);
   void* ptrs[] = {P->d_atom_xyz, P->d_sh_atom, P->d_sh_l, P->d_sh_prim0, P->d_sh_ao0, P->d_prim_alpha, P->d_prim_cn,
-                  P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_ao_atom_c, P->d_x, P->d_fx, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
+                  P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_ao_atom_c, P->d_x, P->d_xd, P->d_fx, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
                   P->d_keys, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_col_ptr, P->d_row_idx, P->d_pos,
                   P->d_blk_amax, P->d_panel_off, P->d_kp, P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
                   P->d_dphi[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,

@@ -435,12 +435,37 @@ def test_nuclear_gradient_parity(K, name, n):
     E2, _ = plan.exc(D, K.KLDI_LDA_SLATER)
     assert abs(E2 - Eref) <= TOL_E
     with pytest.raises(K.KldiError):
-        plan.exc_grad(D, K.KLDI_GGA_PBEX)
+        plan.exc_grad(D, 7)                        # unknown functional
     plan.close()
     plan_lda = K.Plan.from_workload(wl, want_gradients=False)
     with pytest.raises(K.KldiError):
         plan_lda.exc_grad(D)
     plan_lda.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg0", None), ("cfg1", 8), ("cfg2", 6), ("cfg4", 6)])
+def test_nuclear_gradient_gga_parity(K, name, n):
+    """GGA half of SURVEY.md §8(f2): kldi_exc_grad with KLDI_GGA_PBEX (X and X^d = d_d Phi D builds, AO second derivatives
+    on the fly) against the oracle's chain-rule contraction, element by element, same bar; the energy of the same call;
+    the LDA gradient from the same plan afterwards (shared X store)."""
+    import torch
+
+    wl = W.named_config(name, n_override=n, functional="gga")
+    plan = K.Plan.from_workload(wl, want_gradients=True)
+    D = torch.as_tensor(wl.D, device="cuda")
+    E, g = plan.exc_grad(D, K.KLDI_GGA_PBEX)
+    ref = O.exc_nuclear_gradient_gga(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D)
+    Eref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "gga", want_v=False)["E"]
+    g = g.cpu().numpy()
+    assert g.shape == ref.shape == (wl.n_atoms, 3) and np.max(np.abs(ref)) > 1e-3
+    assert np.max(np.abs(g - ref)) <= TOL_GRAD, np.max(np.abs(g - ref))
+    assert abs(E - Eref) <= TOL_E
+    E1, g1 = plan.exc_grad(D, K.KLDI_LDA_SLATER)
+    ref1 = O.exc_nuclear_gradient_lda(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D)
+    assert np.max(np.abs(g1.cpu().numpy() - ref1)) <= TOL_GRAD
+    E2, V = plan.exc(D, K.KLDI_GGA_PBEX)           # the energy / potential path of the same plan is untouched
+    assert abs(E2 - Eref) <= TOL_E
+    plan.close()
 
 
 @pytest.mark.parametrize("n", [4, 44])
