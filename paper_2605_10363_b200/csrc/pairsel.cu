@@ -62,7 +62,10 @@ __global__ void __launch_bounds__(128) k_pair_select(const int32_t* __restrict__
     const int ch0 = cq0 >> 5, ch1 = (cq0 + wq - 1) >> 5;
     for (int ri = lane; ri < (tri ? qi + 1 : ne); ri += 32) {
       const int sr = col_idx[e0 + ri];
-      if (aq * b[(int64_t)sq * n_shells + sr] >= eps) {  // Eq. 17: retain iff a_pq b_qr >= t_d
+      // Eq. 17: retain iff a_pq b_qr >= t_d.  In the triangular form one stage stands for both orientations (q,r) and
+      // (r,q) of the symmetric D, so it runs if EITHER is executable: max(a_pq, a_pr) b_qr >= t_d (a conservative superset)
+      const double aa = tri ? fmax(aq, amax[e0 + ri]) : aq;
+      if (aa * b[(int64_t)sq * n_shells + sr] >= eps) {
         const int cr0 = blk_col0[e0 + ri], wr = sh_ao0[sr + 1] - sh_ao0[sr];
         for (int jt = cr0 / W; jt <= (cr0 + wr - 1) / W; ++jt)
           for (int c = ch0; c <= ch1; ++c) m |= 1ull << (c * 4 + jt);
