@@ -109,6 +109,7 @@ struct kldi_plan {
   double* d_phi = nullptr;         // [total_cols + slack][128] column-major tiles
   double* d_dphi[3] = {nullptr, nullptr, nullptr};
   double* d_phi_v = nullptr;       // second copy of Phi in the V layout (vlayout_off)
+  double* d_dphi_v[3] = {nullptr, nullptr, nullptr};  // gradient stores in the V layout (kldi_build_vtau, first use)
   double* d_z = nullptr;           // GGA: Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, V layout
   double* d_x = nullptr;           // nuclear gradient: X = Phi D of every panel, rho layout, allocated on first use
   double* d_xd = nullptr;          // GGA nuclear gradient: X^d = d_d Phi D, d = x, y, z (three stores) + [n_pad] scratch

@@ -328,7 +328,7 @@ void plan_free(kldi_plan* P) {
                   P->d_shell_perm, P->d_ao_perm, P->d_ao_atom, P->d_ao_atom_c, P->d_x, P->d_xd, P->d_fx, P->d_gx, P->d_gy, P->d_gz, P->d_gw, P->d_perm_g,
                   P->d_keys, P->d_row_ptr, P->d_col_idx, P->d_blk_col0, P->d_col_ptr, P->d_row_idx, P->d_pos,
                   P->d_blk_amax, P->d_panel_off, P->d_kp, P->d_colidx, P->d_phi, P->d_dphi[0], P->d_dphi[1],
-                  P->d_dphi[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
+                  P->d_dphi[2], P->d_dphi_v[0], P->d_dphi_v[1], P->d_dphi_v[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
                   P->d_wv_s, P->d_epart, P->d_E, P->d_stage_host, P->d_vsched_ptr[0], P->d_vsched_ptr[1],
                   P->d_vpasses[0], P->d_vpasses[1], P->d_vitems[0], P->d_vitems[1], P->d_gram_off[0],
                   P->d_gram_off[1], P->d_gram, P->d_ao_shell, P->d_bmax, P->d_pmask, P->d_phiq, P->d_sigma, P->d_Dq, P->d_tau,

@@ -533,19 +533,27 @@ __global__ void __launch_bounds__(128) k_relayout_v(const int64_t* __restrict__ 
 }
 
 // V^tau = 1/2 sum_c (d_c Phi)^T diag(wv) (d_c Phi): three LDA-form Gram builds that accumulate
-// into the same plan-order V; wv_s already carries the 1/2.  Each gradient store is first copied into the V layout
-// (the Z buffer serves as the scratch store).  Mode 1 (workspace + reduce) does not accumulate across launches, so it
-// runs as mode 2 here, which is reproducible and free of FP64 atomics as well.
+// into the same plan-order V; wv_s already carries the 1/2.  The gradient stores are copied into the V layout ONCE, at
+// the first call (the geometry of a plan is fixed), not per call.  Mode 1 (workspace + reduce) does not accumulate across
+// launches, so it runs as mode 2 here, which is reproducible and free of FP64 atomics as well.
 kldi_status launch_vtau(kldi_plan* P) {
   KLDI_CUDA(cudaMemsetAsync(P->d_Vp, 0, sizeof(double) * (size_t)P->n_ao * P->n_ao, P->stream));
   if (P->n_tasks == 0) return KLDI_OK;
   kldi_status rc;
+  if (!P->d_dphi_v[0]) {
+    const size_t tile_bytes = sizeof(double) * GB * (size_t)(P->total_cols + 64);
+    for (int c = 0; c < 3; ++c) {
+      KLDI_CUDA(cudaMalloc(&P->d_dphi_v[c], tile_bytes));
+      KLDI_CUDA(cudaMemsetAsync(P->d_dphi_v[c], 0, tile_bytes, P->stream));
+      k_relayout_v<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_panel_off, P->d_dphi[c], P->d_dphi_v[c]);
+      KLDI_LAUNCHED(P);
+    }
+    P->stats.phi_bytes += 3 * (int64_t)tile_bytes;
+  }
   if (P->v_mode != 0 && (rc = launch_fx_bound(P, false)) != KLDI_OK) return rc;
   for (int c = 0; c < 3; ++c) {
-    k_relayout_v<<<(int)P->n_blocks, 128, 0, P->stream>>>(P->d_panel_off, P->d_dphi[c], P->d_z);
-    KLDI_LAUNCHED(P);
     KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
-    rc = P->v_mode != 0 ? launch_vgram<false, 2>(P, P->d_z) : launch_vgram<false, 0>(P, P->d_z);
+    rc = P->v_mode != 0 ? launch_vgram<false, 2>(P, P->d_dphi_v[c]) : launch_vgram<false, 0>(P, P->d_dphi_v[c]);
     if (rc != KLDI_OK) return rc;
   }
   return KLDI_OK;
