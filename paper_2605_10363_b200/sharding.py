@@ -60,32 +60,29 @@ def curve_order(grid_xyz: np.ndarray) -> np.ndarray:
     return np.argsort(keys, kind="stable")
 
 
-def block_costs(wl, order: np.ndarray, eps: float) -> np.ndarray:
+def block_costs(wl, order: np.ndarray, eps: float, samples_per_block: int = 8) -> np.ndarray:
     """Estimated cost K(K+1) of every 128-point block of the curve order, K = AOs of the shells whose cutoff sphere
-    contains the block's centroid within the block's radius."""
+    contains at least one of `samples_per_block` evenly spaced points of the block (a block far from the molecule is large
+    and sparse: a bounding-sphere test would count every atom there, the plan's filter retains almost nothing)."""
     from scipy.spatial import cKDTree
 
     pts = wl.grid_xyz[order]
     nb = (len(pts) + GB - 1) // GB
-    pad = nb * GB - len(pts)
-    pp = np.vstack([pts, np.repeat(pts[-1:], pad, axis=0)]).reshape(nb, GB, 3) if pad else pts.reshape(nb, GB, 3)
-    cen = pp.mean(axis=1)
-    rad = np.sqrt(((pp - cen[:, None, :]) ** 2).sum(axis=2).max(axis=1))
+    step = GB // samples_per_block
+    sidx = np.arange(0, len(pts), step)
+    sblock = sidx // GB
+    tree = cKDTree(pts[sidx])
     rc = shell_cutoff_radii(wl, eps)
     ncart = np.array([(int(l) + 1) * (int(l) + 2) // 2 for l in wl.shell_l])
     k = np.zeros(nb)
-    tree = cKDTree(cen)
     # group the shells by (atom, cutoff): one ball query per distinct sphere
     by_sphere = {}
     for s in range(len(rc)):
         by_sphere.setdefault((int(wl.shell_atom[s]), round(float(rc[s]), 6)), []).append(s)
-    rmax = float(rad.max()) if nb else 0.0
     for (atom, r), shells in by_sphere.items():
-        w = float(ncart[shells].sum())
-        cand = np.asarray(tree.query_ball_point(wl.atom_xyz[atom], r + rmax), dtype=np.int64)
-        if cand.size:
-            d = np.sqrt(((cen[cand] - wl.atom_xyz[atom]) ** 2).sum(axis=1))
-            k[cand[d <= r + rad[cand]]] += w
+        hit = tree.query_ball_point(wl.atom_xyz[atom], r)
+        if hit:
+            k[np.unique(sblock[np.asarray(hit, dtype=np.int64)])] += float(ncart[shells].sum())
     return k * (k + 1.0)
 
 
