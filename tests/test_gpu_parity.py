@@ -632,6 +632,14 @@ def test_parity_full_size_elementwise(K, name):
     out = run_gpu(K, wl, deterministic_v=2)
     ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, wl.functional, chunk=16384)
     check(out, ref)
+    if wl.functional == "lda":     # the tensor-core rho path on the same full-size workload, same bar
+        import torch
+
+        plan = out["plan"]
+        plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+        D = torch.as_tensor(wl.D, device="cuda")
+        E, V = plan.exc(D)
+        check({"rho": plan.eval_rho(D).cpu().numpy(), "V": V.cpu().numpy(), "E": E, "drho": None}, ref)
     out["plan"].close()
 
 
