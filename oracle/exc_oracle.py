@@ -160,6 +160,13 @@ def vxc_lda_from_wv(phi, wv):
     return phi.T @ (wv[:, None] * phi)
 
 
+def vxc_lda_block_from_wv(phi, wv, rows, cols):
+    """The sub-block V[rows][:, cols] of vxc_lda_from_wv, from the same definition V_{mu,nu} = sum_g wv_g chi_mu chi_nu
+    (Eq. 5) restricted to the wanted AO rows and columns — for stored reference values at sizes where
+    forming all of V on the CPU takes hours (tests/golden/make_cfg3_golden.py)."""
+    return phi[:, rows].T @ (wv[:, None] * phi[:, cols])
+
+
 def vxc_gga_from_wv(phi, dphi, wv4):
     """V = B + B^T, B = Phi^T Z, Z = 1/2 wv0 Phi + sum_c wv_c d_c Phi, with wv0 = w v_rho and
     wv_c = 2 w v_sigma d_c rho (the boundary convention of kldi_build_vxc, include/kldi.h)."""

@@ -131,6 +131,19 @@ def test_ao_gradient_matches_finite_difference(water):
         assert np.max(np.abs(fd - drho[c])) < 1e-7
 
 
+def test_v_block_is_the_block_of_v(water):
+    """vxc_lda_block_from_wv (used for the stored cfg3 reference) is the sub-block of the pinned full V, and one of its
+    entries equals the explicit sum over grid points."""
+    basis = basis_of(water)
+    phi = O.ao_values(*basis, water.grid_xyz)
+    wv = water.grid_w * np.cos(np.arange(water.n_pts))
+    V = O.vxc_lda_from_wv(phi, wv)
+    rows, cols = np.array([0, 7, 24]), np.arange(0, 25, 3)
+    B = O.vxc_lda_block_from_wv(phi, wv, rows, cols)
+    assert B.shape == (3, len(cols)) and np.max(np.abs(B - V[np.ix_(rows, cols)])) < 1e-13
+    assert abs(B[1, 2] - sum(wv[g] * phi[g, 7] * phi[g, 6] for g in range(water.n_pts))) < 1e-12
+
+
 def test_nuclear_gradient_lda_matches_finite_difference_of_energy(water):
     """the paper prints no gradient formula, so the oracle's EXC nuclear-gradient contraction is
     pinned by central differences of the (closed-form-pinned) energy in the atom coordinates, grid held fixed, and
