@@ -274,6 +274,20 @@ kldi_status kldi_ao_order(const kldi_atoms* atoms, const kldi_shells* shells, in
 typedef enum { KLDI_DEFAULT_AO_ORDER = 1 } kldi_plan_default;
 kldi_status kldi_set_plan_default(kldi_plan_default what, int value);
 
+/* The functional + energy step without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture,
+ * serving loops, harnesses that forbid it): Slater exchange per point, spin-restricted (Eq. 1, 71 Eq. 3),
+ *     wv[g] = w[g] v_rho(rho[g]),   *Exc_dev = sum_g w[g] e(rho[g]),   e = v = 0 where rho < 1e-20,
+ * the same arithmetic as the functional stage of kldi_exc (a fixed reduction tree: bitwise reproducible).  No plan:
+ * rho, w, wv DEVICE [n_pts] in one common point order, Exc_dev DEVICE one value; asynchronous on cuda_stream (a
+ * cudaStream_t, NULL = default stream) of the CURRENT device.  The per-block partial sums live in a static device array
+ * of the library (256 KB, held by every GPU that loads the library until exit), hence the limit
+ * n_pts <= kldi_xc_lda_noalloc_max_pts() = 8,388,608: larger -> KLDI_EINVAL.  Calls no cudaMalloc / cudaFree.  Every call
+ * on a device shares that array: it keeps the last call's contents (each call overwrites what it then reads), and calls
+ * that overlap on the GPU (different streams, or graphs replayed concurrently) race on it. */
+kldi_status kldi_xc_lda_noalloc(const double* rho, const double* w, int64_t n_pts, double* wv, double* Exc_dev,
+                                void* cuda_stream);
+int64_t kldi_xc_lda_noalloc_max_pts(void);
+
 const char* kldi_last_error(void);
 
 #ifdef __cplusplus

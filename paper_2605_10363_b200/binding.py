@@ -22,7 +22,8 @@ EXPORTED = [
     "kldi_plan_create", "kldi_plan_destroy", "kldi_plan_stats", "kldi_eval_rho", "kldi_build_vxc", "kldi_exc",
     "kldi_exc_host", "kldi_exc_grad", "kldi_eval_tau", "kldi_build_vtau", "kldi_last_timings", "kldi_plan_export", "kldi_plan_export_tile", "kldi_fp64_peak",
     "kldi_morton_key", "kldi_grid_key", "kldi_grid_keys", "kldi_last_error", "kldi_plan_set_option", "kldi_vsched_export",
-    "kldi_vlayout_offset", "kldi_ao_order", "kldi_set_plan_default",
+    "kldi_vlayout_offset", "kldi_ao_order", "kldi_set_plan_default", "kldi_xc_lda_noalloc",
+    "kldi_xc_lda_noalloc_max_pts",
 ]
 KLDI_OPT_DETERMINISTIC_V = 1
 KLDI_OPT_PAIR_TEST = 2
@@ -101,11 +102,15 @@ def lib():
         L.kldi_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.kldi_ao_order.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.kldi_set_plan_default.argtypes = [C.c_int, C.c_int]
+        L.kldi_xc_lda_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.kldi_xc_lda_noalloc_max_pts.argtypes = []
+        L.kldi_xc_lda_noalloc_max_pts.restype = C.c_int64
         L.kldi_vsched_export.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.kldi_vlayout_offset.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         L.kldi_vlayout_offset.restype = C.c_int64
         for name in EXPORTED:
-            if name not in ("kldi_last_error", "kldi_morton_key", "kldi_grid_key", "kldi_vlayout_offset"):
+            if name not in ("kldi_last_error", "kldi_morton_key", "kldi_grid_key", "kldi_vlayout_offset",
+                            "kldi_xc_lda_noalloc_max_pts"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -325,6 +330,26 @@ def ao_order(atom_xyz, shell_atom, shell_l, shell_prim_off, prim_alpha, prim_coe
     _check(lib().kldi_ao_order(C.byref(atoms), C.byref(shells), 1, C.c_void_p(order.ctypes.data),
                                C.c_void_p(dist.ctypes.data) if want_dist else None), "kldi_ao_order")
     return (order, dist) if want_dist else order
+
+
+def xc_lda_noalloc(rho, w, wv_out, E_out, stream=None) -> None:
+    """kldi_xc_lda_noalloc: wv_out = w v_rho(rho), E_out[0] = sum w e(rho); all four are float64 CUDA tensors the caller
+    owns ([n], [n], [n], [1]); nothing is allocated.  Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+
+    n = rho.numel()
+    for t, m in ((rho, n), (w, n), (wv_out, n), (E_out, 1)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.numel() == m):
+            raise KldiError("xc_lda_noalloc: expected contiguous float64 CUDA tensors of sizes n, n, n, 1")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().kldi_xc_lda_noalloc(C.c_void_p(rho.data_ptr()), C.c_void_p(w.data_ptr()), n,
+                                     C.c_void_p(wv_out.data_ptr()), C.c_void_p(E_out.data_ptr()),
+                                     C.c_void_p(st.cuda_stream)), "kldi_xc_lda_noalloc")
+
+
+def xc_lda_noalloc_max_pts() -> int:
+    return int(lib().kldi_xc_lda_noalloc_max_pts())
 
 
 def grid_keys(xyz, origin) -> np.ndarray:

@@ -40,7 +40,7 @@ def _newer(target: str, sources: list) -> bool:
 
 
 def build_kldi(force: bool = False, verbose: bool = False) -> str:
-    srcs = [os.path.join(CSRC, f) for f in ("api.cu", "plan.cu", "contract.cu", "vgram.cu", "pairsel.cu", "rho_i8.cu", "aoorder.cu")]
+    srcs = [os.path.join(CSRC, f) for f in ("api.cu", "plan.cu", "contract.cu", "vgram.cu", "pairsel.cu", "rho_i8.cu", "aoorder.cu", "xc_noalloc.cu")]
     deps = srcs + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))]
     deps.append(os.path.join(ROOT, "include", "kldi.h"))
     if not force and _newer(LIB, deps):
