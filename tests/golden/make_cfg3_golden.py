@@ -15,7 +15,10 @@ all of V, so the script walks the grid in chunks and takes the oracle's own step
 tests/test_oracle_pins.py.)  The Becke partition of the 4.2 M points (2.5e12 cell functions) is input generation, not
 method arithmetic; pass the weights the same generator wrote on a GPU box with `--weights cfg3_w.npy` (workloads/becke.cu;
 tests/test_gpu_parity.py::test_becke_cuda_equals_numpy holds it to the numpy recipe), or omit it to run the numpy Becke
-(days).  The run is resumable: a checkpoint is written every `--sub` points and a later invocation continues from it.
+(days).  The run is resumable: a checkpoint is written every `--sub` points and a later invocation continues from it;
+`--lo/--hi` restrict a run to a range of points (every stored quantity is a sum over points or a per-point value), so that
+disjoint ranges can run on different machines, and `--merge a.ckpt.npz b.ckpt.npz ...` adds finished ranges that tile
+[0, n_pts) into the final file.
 
 Stored (all float64): E; rho and wv on every 64th point; 16 full rows of V and the strided sample V[::97, ::89]; sum and
 sum of squares of the weights (so that a test can tell that it runs on the same inputs).
@@ -49,6 +52,9 @@ def main():
     ap.add_argument("--sub", type=int, default=262144, help="points per checkpoint")
     ap.add_argument("--checkpoint", default=None, help="checkpoint file (default: <out>.ckpt.npz)")
     ap.add_argument("--budget", type=float, default=0.0, help="stop after this many seconds (0 = run to the end)")
+    ap.add_argument("--lo", type=int, default=0, help="first point of this run's range")
+    ap.add_argument("--hi", type=int, default=-1, help="end of this run's range (default: all points)")
+    ap.add_argument("--merge", nargs="+", default=None, help="checkpoints of finished ranges that tile [0, n_pts)")
     a = ap.parse_args()
     gw = np.load(a.weights) if a.weights else None
     wl = W.named_config(a.config, grid_w=gw, becke_backend="numpy")
@@ -59,20 +65,36 @@ def main():
     allc = np.arange(n_ao)
     sr, sc = np.arange(0, n_ao, STRIDE_V[0]), np.arange(0, n_ao, STRIDE_V[1])
     ck = a.checkpoint or (a.out + ".ckpt.npz")
-    if os.path.exists(ck):
+    r_lo, r_hi = a.lo, (n if a.hi < 0 else min(n, a.hi))
+    if a.merge:
+        parts = [dict(np.load(f)) for f in a.merge]
+        parts.sort(key=lambda d: int(d.get("lo", 0)))
+        edge = 0
+        for d in parts:   # the ranges must tile [0, n) without gap or overlap; `done` may be cut back to the next range's lo
+            assert int(d["n_pts"]) == n and abs(float(d["w_sum"]) - wl.grid_w.sum()) <= 1e-9 * abs(wl.grid_w.sum())
+            assert int(d.get("lo", 0)) == edge and int(d["done"]) > edge, (int(d.get("lo", 0)), edge)
+            edge = int(d["done"])
+        assert edge == n, (edge, n)
+        st = {"done": np.int64(n), "seconds": np.float64(sum(float(d["seconds"]) for d in parts)),
+              "E_parts": np.concatenate([d["E_parts"] for d in parts]),
+              "rho_max": np.float64(max(float(d["rho_max"]) for d in parts))}
+        for k in ("rho_strided", "wv_strided", "V_rows", "V_strided"):
+            st[k] = sum(d[k] for d in parts)
+    elif os.path.exists(ck):
         z = np.load(ck)
         st = {k: z[k] for k in z.files}
         assert int(st["n_pts"]) == n and abs(float(st["w_sum"]) - wl.grid_w.sum()) <= 1e-9 * abs(wl.grid_w.sum())
         print(f"resuming from {ck}: {int(st['done'])} of {n} points done", flush=True)
     else:
-        st = {"done": np.int64(0), "n_pts": np.int64(n), "w_sum": np.float64(wl.grid_w.sum()), "E_parts": np.zeros(0),
+        st = {"done": np.int64(r_lo), "lo": np.int64(r_lo), "n_pts": np.int64(n), "w_sum": np.float64(wl.grid_w.sum()),
+              "E_parts": np.zeros(0),
               "rho_strided": np.zeros((n + sp - 1) // sp), "wv_strided": np.zeros((n + sp - 1) // sp),
               "V_rows": np.zeros((len(rows), n_ao)), "V_strided": np.zeros((len(sr), len(sc))),
               "rho_max": np.float64(0.0), "seconds": np.float64(0.0)}
     t_start = time.time()
-    while int(st["done"]) < n and (a.budget <= 0 or time.time() - t_start < a.budget):
+    while not a.merge and int(st["done"]) < r_hi and (a.budget <= 0 or time.time() - t_start < a.budget):
         lo = int(st["done"])
-        hi = min(n, lo + a.sub)
+        hi = min(r_hi, lo + a.sub)
         t0 = time.time()
         e_terms = []
         for c0 in range(lo, hi, a.chunk):
@@ -94,8 +116,8 @@ def main():
         np.savez(ck + ".tmp.npz", **st)
         os.replace(ck + ".tmp.npz", ck)
         print(f"  points {lo}..{hi} of {n}: {time.time() - t0:.0f} s", flush=True)
-    if int(st["done"]) < n:
-        print(f"budget reached at {int(st['done'])} of {n} points; run again to continue from {ck}")
+    if not a.merge and (int(st["done"]) < n or r_lo > 0):
+        print(f"range {r_lo}..{r_hi}: {int(st['done'])} reached; checkpoint {ck} (run again to continue, or --merge)")
         return
     E = math.fsum(st["E_parts"].tolist())
     np.savez(a.out, E=np.float64(E), rho_strided=st["rho_strided"], wv_strided=st["wv_strided"],
