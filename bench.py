@@ -198,7 +198,16 @@ def main():
     from paper_2605_10363_b200 import workloads as W
 
     t0 = time.perf_counter()
-    wl_full = W.named_config(args.config, eps=args.eps)
+    if world == 1:
+        wl_full = W.named_config(args.config, eps=args.eps)
+    else:
+        # the Becke partition (2.5e12 cell functions on cfg3) is evaluated once, on rank 0, and its weights broadcast;
+        # geometry, basis, grid points and D are cheap and seeded, every rank builds them itself
+        wl_full = W.named_config(args.config, eps=args.eps, becke_backend="auto" if rank == 0 else "none")
+        gw = torch.as_tensor(wl_full.grid_w, device="cuda").contiguous()
+        dist.broadcast(gw, src=0)
+        wl_full.grid_w = gw.cpu().numpy()
+        del gw
     gen_s = time.perf_counter() - t0
     wl = wl_full
     if world > 1:
