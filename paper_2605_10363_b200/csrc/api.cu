@@ -387,8 +387,12 @@ kldi_status kldi_eval_tau(kldi_plan* P, const double* D, double* tau) {
   EV(0);
   if ((rc = launch_permute_D(P, D, false)) != KLDI_OK) return rc;  // triangular D': the product is symmetric in mu, nu
   EV(1);
-  for (int c = 0; c < 3; ++c)
-    if ((rc = launch_rho_lda_on(P, P->d_dphi[c], P->d_drho_s + (size_t)c * P->n_pad)) != KLDI_OK) return rc;
+  if (P->rho_impl == 2) {  // KLDI_OPT_RHO_TC: the three builds as int8 slice products on tcgen05
+    if ((rc = launch_tau_tc(P)) != KLDI_OK) return rc;
+  } else {
+    for (int c = 0; c < 3; ++c)
+      if ((rc = launch_rho_lda_on(P, P->d_dphi[c], P->d_drho_s + (size_t)c * P->n_pad)) != KLDI_OK) return rc;
+  }
   if ((rc = launch_tau_combine(P)) != KLDI_OK) return rc;
   EV(2);
   if ((rc = launch_unpermute_rho(P, tau, nullptr)) != KLDI_OK) return rc;

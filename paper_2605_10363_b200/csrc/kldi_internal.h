@@ -128,6 +128,8 @@ struct kldi_plan {
   // ---- int8 slice-product path (rho_i8.cu), allocated on first use
   unsigned char* d_phiq = nullptr;                // [tc_chunks][NSL][4096] digit planes of Phi, tensor-core smem image
   double* d_sigma = nullptr;                      // [n_pad] row scales of the digit planes
+  unsigned char* d_dphiq[3] = {nullptr, nullptr, nullptr};  // the same for the gradient stores (kldi_eval_tau, first use)
+  double* d_dsigma[3] = {nullptr, nullptr, nullptr};
   unsigned long long* d_Dq = nullptr;             // [n_ao][n_ao] packed digits of D' (per call)
   double* d_tau = nullptr;                        // [2][n_ao] column scales of D', column maxima
   int64_t* d_chunk_off = nullptr;                 // [n_blocks+1] first 32-column chunk of grid block p
@@ -182,6 +184,7 @@ kldi_status launch_x_on(kldi_plan* P, const double* store, double* x_out, double
 kldi_status launch_grad_cols_gga(kldi_plan* P, double* grad);
 // rho_i8.cu
 kldi_status launch_rho_tc(kldi_plan* P);
+kldi_status launch_tau_tc(kldi_plan* P);  // t_c = rowsum(d_c Phi o d_c Phi D') for c = x, y, z into d_drho_s (D' in d_Dp)
 kldi_status launch_grad_cols(kldi_plan* P, double* grad);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);

@@ -331,7 +331,8 @@ void plan_free(kldi_plan* P) {
                   P->d_dphi[2], P->d_dphi_v[0], P->d_dphi_v[1], P->d_dphi_v[2], P->d_z, P->d_phi_v, P->d_tasks, P->d_ticket, P->d_Dp, P->d_Vp, P->d_rho_s, P->d_drho_s,
                   P->d_wv_s, P->d_epart, P->d_E, P->d_stage_host, P->d_vsched_ptr[0], P->d_vsched_ptr[1],
                   P->d_vpasses[0], P->d_vpasses[1], P->d_vitems[0], P->d_vitems[1], P->d_gram_off[0],
-                  P->d_gram_off[1], P->d_gram, P->d_ao_shell, P->d_bmax, P->d_pmask, P->d_phiq, P->d_sigma, P->d_Dq, P->d_tau,
+                  P->d_gram_off[1], P->d_gram, P->d_ao_shell, P->d_bmax, P->d_pmask, P->d_phiq, P->d_sigma, P->d_dphiq[0], P->d_dphiq[1], P->d_dphiq[2], P->d_dsigma[0], P->d_dsigma[1],
+                  P->d_dsigma[2], P->d_Dq, P->d_tau,
                   P->d_chunk_off};
   for (void* q : ptrs)
     if (q) cudaFree(q);

@@ -492,7 +492,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 // ------------------------------------------------------------------------------------------------ host side
 template <int NSL>
 static kldi_status tc_prepare(kldi_plan* P) {
-  if (P->d_phiq) return KLDI_OK;
+  if (P->d_chunk_off) return KLDI_OK;
   if (P->stats.max_k > 16384) {
     set_error("KLDI_OPT_RHO_TC: a grid block retains %lld AO columns; the int32 accumulators hold 16384", (long long)P->stats.max_k);
     return KLDI_ESTATE;
@@ -522,32 +522,33 @@ static kldi_status tc_prepare(kldi_plan* P) {
     }
     P->stats.ops_rho_tc = ops;
   }
-  KLDI_CUDA(cudaMalloc(&P->d_chunk_off, sizeof(int64_t) * (P->n_blocks + 1)));
-  KLDI_CUDA(cudaMemcpyAsync(P->d_chunk_off, h_chunk.data(), sizeof(int64_t) * (P->n_blocks + 1), cudaMemcpyHostToDevice, P->stream));
-  KLDI_CUDA(cudaStreamSynchronize(P->stream));  // h_chunk goes out of scope
-  KLDI_CUDA(cudaMalloc(&P->d_sigma, sizeof(double) * P->n_pad));
-  KLDI_CUDA(cudaMalloc(&P->d_phiq, (size_t)std::max<int64_t>(1, P->tc_chunks) * NSL * tc::A_SLICE));
   KLDI_CUDA(cudaMalloc(&P->d_Dq, sizeof(unsigned long long) * (size_t)P->n_ao * P->n_ao));
   KLDI_CUDA(cudaMemsetAsync(P->d_Dq, 0, sizeof(unsigned long long) * (size_t)P->n_ao * P->n_ao, P->stream));
   KLDI_CUDA(cudaMalloc(&P->d_tau, sizeof(double) * 2 * P->n_ao));
+  KLDI_CUDA(cudaMalloc(&P->d_chunk_off, sizeof(int64_t) * (P->n_blocks + 1)));
+  KLDI_CUDA(cudaMemcpyAsync(P->d_chunk_off, h_chunk.data(), sizeof(int64_t) * (P->n_blocks + 1), cudaMemcpyHostToDevice, P->stream));
+  KLDI_CUDA(cudaStreamSynchronize(P->stream));  // h_chunk goes out of scope
+  return ensure_smem_attr((const void*)tc::k_rho_i8<NSL>, tc::Cfg<NSL>::SMEM_BYTES, P->device);
+}
+
+// Digit planes and row scales of one store of the rho layout (Phi or a gradient store), once per plan.
+template <int NSL>
+static kldi_status tc_prepare_store(kldi_plan* P, const double* store, unsigned char** planes, double** scales) {
+  if (*planes) return KLDI_OK;
+  KLDI_CUDA(cudaMalloc(scales, sizeof(double) * P->n_pad));
+  KLDI_CUDA(cudaMalloc(planes, (size_t)std::max<int64_t>(1, P->tc_chunks) * NSL * tc::A_SLICE));
   if (P->n_tasks > 0) {
-    tc::k_slice_phi<NSL><<<P->n_tasks, 128, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_phi,
-                                                           P->d_sigma, P->d_phiq);
+    tc::k_slice_phi<NSL><<<P->n_tasks, 128, 0, P->stream>>>(P->d_tasks, P->d_kp, P->d_panel_off, P->d_chunk_off, store,
+                                                           *scales, *planes);
     KLDI_LAUNCHED(P);
   }
   P->stats.phi_bytes += (int64_t)P->tc_chunks * NSL * tc::A_SLICE;
   return KLDI_OK;
 }
 
-// rho_s of every grid block from D' in P->d_Dp (written by launch_permute_D in its triangular form).
-kldi_status launch_rho_tc(kldi_plan* P) {
-  constexpr int NSL = 5;
-  kldi_status rc = tc_prepare<NSL>(P);
-  if (rc != KLDI_OK) return rc;
-  if ((rc = ensure_smem_attr((const void*)tc::k_rho_i8<NSL>, tc::Cfg<NSL>::SMEM_BYTES, P->device)) != KLDI_OK) return rc;
-  KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
-  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
-  if (P->n_tasks == 0) return KLDI_OK;
+// The digits and column scales of D' (in P->d_Dp, triangular form), once per call.
+template <int NSL>
+static kldi_status tc_slice_D(kldi_plan* P) {
   const int n = P->n_ao;
   double* cmax = P->d_tau + n;
   KLDI_CUDA(cudaMemsetAsync(cmax, 0, sizeof(double) * n, P->stream));
@@ -555,6 +556,15 @@ kldi_status launch_rho_tc(kldi_plan* P) {
   KLDI_LAUNCHED(P);
   tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq);
   KLDI_LAUNCHED(P);
+  return KLDI_OK;
+}
+
+// out_s[g] = 2 sum_{mu >= nu} D'_{mu,nu} A_{g,mu} A_{g,nu} for the store A (FP64 columns `store`, digit planes `planes`)
+template <int NSL>
+static kldi_status tc_contract(kldi_plan* P, const double* store, const unsigned char* planes, const double* scales,
+                               double* out_s) {
+  KLDI_CUDA(cudaMemsetAsync(out_s, 0, sizeof(double) * P->n_pad, P->stream));
+  KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
   static const bool debug = getenv("KLDI_TC_DEBUG") != nullptr;  // per-role wait cycles, printed to stderr (synchronises)
   long long* dbg = nullptr;
@@ -563,8 +573,8 @@ kldi_status launch_rho_tc(kldi_plan* P) {
     KLDI_CUDA(cudaMemsetAsync(dbg, 0, 32 * sizeof(long long), P->stream));
   }
   tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
-      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, P->d_phi, P->d_phiq,
-      P->d_sigma, P->d_Dq, P->d_tau, n, P->d_rho_s, dbg);
+      P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, store, planes, scales,
+      P->d_Dq, P->d_tau, P->n_ao, out_s, dbg);
   KLDI_LAUNCHED(P);
   if (debug) {
     long long h[32];
@@ -580,6 +590,39 @@ kldi_status launch_rho_tc(kldi_plan* P) {
       fprintf(stderr, "  (cycles per warp)\n");
     }
   }
+  return KLDI_OK;
+}
+
+constexpr int TC_NSL = 5;
+
+// rho_s of every grid block from D' in P->d_Dp (written by launch_permute_D in its triangular form).
+kldi_status launch_rho_tc(kldi_plan* P) {
+  kldi_status rc = tc_prepare<TC_NSL>(P);
+  if (rc != KLDI_OK) return rc;
+  if ((rc = tc_prepare_store<TC_NSL>(P, P->d_phi, &P->d_phiq, &P->d_sigma)) != KLDI_OK) return rc;
+  if (P->n_tasks == 0) {
+    KLDI_CUDA(cudaMemsetAsync(P->d_rho_s, 0, sizeof(double) * P->n_pad, P->stream));
+    return KLDI_OK;
+  }
+  if ((rc = tc_slice_D<TC_NSL>(P)) != KLDI_OK) return rc;
+  return tc_contract<TC_NSL>(P, P->d_phi, P->d_phiq, P->d_sigma, P->d_rho_s);
+}
+
+// The three LDA-form builds of the kinetic-energy density on the gradient stores, D' split once.
+kldi_status launch_tau_tc(kldi_plan* P) {
+  kldi_status rc = tc_prepare<TC_NSL>(P);
+  if (rc != KLDI_OK) return rc;
+  for (int c = 0; c < 3; ++c)
+    if ((rc = tc_prepare_store<TC_NSL>(P, P->d_dphi[c], &P->d_dphiq[c], &P->d_dsigma[c])) != KLDI_OK) return rc;
+  if (P->n_tasks == 0) {
+    KLDI_CUDA(cudaMemsetAsync(P->d_drho_s, 0, sizeof(double) * 3 * P->n_pad, P->stream));
+    return KLDI_OK;
+  }
+  if ((rc = tc_slice_D<TC_NSL>(P)) != KLDI_OK) return rc;
+  for (int c = 0; c < 3; ++c)
+    if ((rc = tc_contract<TC_NSL>(P, P->d_dphi[c], P->d_dphiq[c], P->d_dsigma[c], P->d_drho_s + (size_t)c * P->n_pad)) !=
+        KLDI_OK)
+      return rc;
   return KLDI_OK;
 }
 

@@ -521,6 +521,13 @@ def test_tau_and_vtau_parity(K, name, n, mode):
     if mode == 2:
         V2 = plan.build_vtau(torch.as_tensor(wv, device="cuda"))
         assert torch.equal(V2, Vt)
+    if mode == 2:   # kldi_eval_tau follows KLDI_OPT_RHO_TC (three int8 slice-product builds on the gradient stores)
+        plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+        tau_tc = plan.eval_tau(D)
+        tau_tc2 = plan.eval_tau(D)
+        assert np.max(np.abs(tau_tc.cpu().numpy() - tau_ref)) <= TOL_RHO
+        assert torch.equal(tau_tc, tau_tc2)
+        plan.set_option(K.KLDI_OPT_RHO_TC, 0)
     # the energy / potential path of the same plan is untouched by the scratch use of the Z store
     E, V = plan.exc(D, K.KLDI_GGA_PBEX)
     ref = O.exc(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D, "gga")
