@@ -220,8 +220,9 @@ kldi_status kldi_exc_grad(kldi_plan* plan, const double* D, kldi_functional f, d
  * >= 256^-6 are accumulated exactly, and rho is recombined in FP64.  Error ~1e-10 absolute on rho (same parity bar,
  * 1e-9); rho stays bitwise reproducible.  Costs a second store of 5 bytes per retained Phi value and n_ao^2 64-bit
  * words.  kldi_eval_tau follows the option too (its three builds on the gradient stores; three more digit stores).
- * Ignored for GGA, while KLDI_OPT_PAIR_TEST is on, and by kldi_exc_grad; KLDI_ESTATE from the compute call if a grid
- * block retains more than 16384 AO columns.
+ * kldi_exc_grad runs its X-only builds (LDA: X = Phi D; GGA: the three X^d = d_d Phi D; full D) the same way.  Ignored by
+ * the GGA rho contraction of kldi_exc / kldi_eval_rho and while KLDI_OPT_PAIR_TEST is on; KLDI_ESTATE from the compute
+ * call if a grid block retains more than 16384 AO columns.
  * KLDI_OPT_HOST_V_TRIANGLE: 0 (default) = kldi_exc_host fills all of V_host; 1 = only its lower triangle (row >= column,
  * the convention D is read in), in row bands: V is exactly symmetric, so the other half is redundant and the
  * device-to-host copy halves. */

@@ -450,11 +450,20 @@ kldi_status kldi_exc_grad(kldi_plan* P, const double* D, kldi_functional f, doub
   if ((rc = launch_permute_D(P, D, true)) != KLDI_OK) return rc;  // full D: the gradient needs X = Phi D itself
   EV(1);
   // LDA: X-only form (rho + X).  GGA: the GGA form (rho, grad rho and X in one pass), then X^d = d_d Phi D
-  if ((rc = launch_rho(P, true, P->d_x, !gga)) != KLDI_OK) return rc;
+  // KLDI_OPT_RHO_TC: the X-only builds (LDA: X = Phi D; GGA: the three X^d) run as int8 slice products on tcgen05
+  const bool tc = P->rho_impl == 2 && !P->pair_test;
+  if (!gga && tc) {
+    if ((rc = launch_x_tc(P, 0, P->d_x, P->d_rho_s, true)) != KLDI_OK) return rc;
+  } else if ((rc = launch_rho(P, true, P->d_x, !gga)) != KLDI_OK) {
+    return rc;
+  }
   if (gga) {
     double* scratch = P->d_xd + 3 * (store / sizeof(double));
-    for (int d = 0; d < 3; ++d)
-      if ((rc = launch_x_on(P, P->d_dphi[d], P->d_xd + d * (store / sizeof(double)), scratch)) != KLDI_OK) return rc;
+    for (int d = 0; d < 3; ++d) {
+      double* xd = P->d_xd + d * (store / sizeof(double));
+      rc = tc ? launch_x_tc(P, 1 + d, xd, scratch, d == 0) : launch_x_on(P, P->d_dphi[d], xd, scratch);
+      if (rc != KLDI_OK) return rc;
+    }
   }
   EV(2);
   if ((rc = launch_xc(P, f)) != KLDI_OK) return rc;

@@ -130,6 +130,7 @@ struct kldi_plan {
   double* d_sigma = nullptr;                      // [n_pad] row scales of the digit planes
   unsigned char* d_dphiq[3] = {nullptr, nullptr, nullptr};  // the same for the gradient stores (kldi_eval_tau, first use)
   double* d_dsigma[3] = {nullptr, nullptr, nullptr};
+  bool dq_upper_dirty = false;                    // the last digit split wrote the upper triangle of Dq (full-D form)
   unsigned long long* d_Dq = nullptr;             // [n_ao][n_ao] packed digits of D' (per call)
   double* d_tau = nullptr;                        // [2][n_ao] column scales of D', column maxima
   int64_t* d_chunk_off = nullptr;                 // [n_blocks+1] first 32-column chunk of grid block p
@@ -184,7 +185,8 @@ kldi_status launch_x_on(kldi_plan* P, const double* store, double* x_out, double
 kldi_status launch_grad_cols_gga(kldi_plan* P, double* grad);
 // rho_i8.cu
 kldi_status launch_rho_tc(kldi_plan* P);
-kldi_status launch_tau_tc(kldi_plan* P);  // t_c = rowsum(d_c Phi o d_c Phi D') for c = x, y, z into d_drho_s (D' in d_Dp)
+kldi_status launch_tau_tc(kldi_plan* P);
+kldi_status launch_x_tc(kldi_plan* P, int which, double* x_out, double* rho_out, bool slice_d);  // t_c = rowsum(d_c Phi o d_c Phi D') for c = x, y, z into d_drho_s (D' in d_Dp)
 kldi_status launch_grad_cols(kldi_plan* P, double* grad);
 kldi_status launch_unpermute_rho(kldi_plan* P, double* rho, double* drho);
 kldi_status launch_xc(kldi_plan* P, kldi_functional f);

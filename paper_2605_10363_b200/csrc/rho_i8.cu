@@ -105,10 +105,11 @@ __global__ void __launch_bounds__(128) k_slice_phi(const int32_t* __restrict__ t
 // ------------------------------------------------------------------------------------------------ per call
 // tau_n = max_k |D'(k,n)| * 256/127 over the stored (lower-triangular, plan-order) D'.  Non-negative doubles order like
 // their bit patterns, so the column maximum is an integer atomicMax.
-__global__ void __launch_bounds__(256) k_colmax(const double* __restrict__ Dp, int n, unsigned long long* __restrict__ mx) {
+__global__ void __launch_bounds__(256) k_colmax(const double* __restrict__ Dp, int n, unsigned long long* __restrict__ mx,
+                                                int tri) {
   const int j = blockIdx.x * 32 + (threadIdx.x & 31);
   const int r0 = blockIdx.y * 256 + (threadIdx.x >> 5);
-  if (j >= n || blockIdx.y * 256 + 255 < blockIdx.x * 32) return;  // rows above the diagonal hold zeros
+  if (j >= n || (tri && blockIdx.y * 256 + 255 < blockIdx.x * 32)) return;  // tri: rows above the diagonal hold zeros
   double m = 0.0;
   for (int r = r0; r < min(n, blockIdx.y * 256 + 256); r += 8) m = fmax(m, fabs(Dp[(int64_t)r * n + j]));
   if (m > 0.0) atomicMax(mx + j, (unsigned long long)__double_as_longlong(m));
@@ -118,15 +119,16 @@ __global__ void __launch_bounds__(256) k_colmax(const double* __restrict__ Dp, i
 // tau[n] is rewritten in place from the maximum to the scale.
 template <int NSL>
 __global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, int n, const double* __restrict__ cmax,
-                                                 double* __restrict__ tau, unsigned long long* __restrict__ Dq) {
+                                                 double* __restrict__ tau, unsigned long long* __restrict__ Dq, int tri) {
   const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y;
   if (j >= n) return;
-  if (blockIdx.x * 256 > i && i > 0) return;  // strictly above the diagonal: Dq was zeroed once and is never written there
+  // tri: strictly above the diagonal Dq was zeroed and is never written (a full-D call marks it dirty, tc_slice_D)
+  if (tri && blockIdx.x * 256 > i && i > 0) return;
   const double m = cmax[j];
   const double t = m > 0.0 ? m * (256.0 / 127.0) : 1.0;
   if (i == 0) tau[j] = t;
   unsigned long long q = 0;
-  if (j <= i) {
+  if (!tri || j <= i) {
     long long v = __double2ll_rn(Dp[(int64_t)i * n + j] * scalbn(1.0 / t, 8 * NSL));
 #pragma unroll
     for (int s = NSL - 1; s >= 0; --s) {
@@ -159,13 +161,13 @@ __global__ void __launch_bounds__(256) k_slice_D(const double* __restrict__ Dp, 
 // only its columns n < k0 + 32; the chunks are walked in DESCENDING k0, so the first one is full width and overwrites
 // (zeroes) every accumulator column of the tile.  The five accumulator classes of a 96-column tile fill tensor memory
 // (480 of 512 columns), so the MMAs of a tile and the epilogue of the previous one alternate.
-template <int NSL>
+template <int NSL, bool XOUT>
 __global__ void __launch_bounds__(NTHREADS, 1)
     k_rho_i8(const int32_t* __restrict__ tasks, int n_tasks, int32_t* __restrict__ ticket, const int32_t* __restrict__ kp,
              const int64_t* __restrict__ panel_off, const int64_t* __restrict__ chunk_off,
              const int32_t* __restrict__ colidx, const double* __restrict__ phi, const unsigned char* __restrict__ phiq,
              const double* __restrict__ sigma, const unsigned long long* __restrict__ Dq, const double* __restrict__ tau,
-             int n_ao, double* __restrict__ rho_s, long long* __restrict__ dbg) {
+             int n_ao, double* __restrict__ rho_s, double* __restrict__ x_out, long long* __restrict__ dbg) {
   using C = Cfg<NSL>;
   extern __shared__ __align__(128) unsigned char smem[];
   long long tw[6] = {0, 0, 0, 0, 0, 0};  // debug: cycles spent in the waits of this warp's role
@@ -228,7 +230,9 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           const int n = n0 + lane + 32 * u;
           cn[u] = (lane + 32 * u < Wj && n < K8) ? colidx[base + n] : -1;
         }
-        for (int k0 = K32 - KC; k0 >= n0; k0 -= KC) {
+        // XOUT (X = A D with the FULL D, the X builds of the nuclear gradient): every chunk reaches every tile
+        const int kmin = XOUT ? 0 : n0;
+        for (int k0 = K32 - KC; k0 >= kmin; k0 -= KC) {
           const int s = t % NST;
           const int k = k0 + lane;
           const int kr = k < K8 ? colidx[base + k] : -1;
@@ -242,8 +246,8 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           if (lane == 0) {
             int fl = 0;
             if (k0 == K32 - KC) fl |= F_FIRST;
-            if (k0 == n0) fl |= F_LAST_TILE | (jt == ntile - 1 ? F_LAST_PANEL : 0);
-            const int wact = min(Wj, k0 + KC - n0);
+            if (k0 == kmin) fl |= F_LAST_TILE | (jt == ntile - 1 ? F_LAST_PANEL : 0);
+            const int wact = XOUT ? Wj : min(Wj, k0 + KC - n0);
             hdr[4 * s + 0] = p;
             hdr[4 * s + 1] = n0 | (k0 << 16);
             hdr[4 * s + 2] = fl | (wact << 8) | (Wj << 16) | ((tile & 3) << 24);
@@ -422,13 +426,22 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       tc_fence_after();
       const long long t_e0 = dbg ? clock64() : 0;
       double rs2 = 0.0;
+      double xs = 0.0;
+      double* xg = nullptr;
+      if (XOUT) {
+        xs = scalbn(sigma[(int64_t)p * GB + g], -8 * (NSL + 1));
+        xg = x_out + (panel_off[p] + n0) * GB + g;
+      }
       for (int j0 = 8 * hs; j0 < wj; j0 += 8 * NSET) {
         int32_t acc[NSL][8];
 #pragma unroll
         for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
-        double f[8];  // tau_n Phi(g,n) of the columns j0 .. j0+7
+        double f[8], tj[8];  // tau_n Phi(g,n) of the columns j0 .. j0+7
 #pragma unroll
-        for (int j = 0; j < 8; ++j) f[j] = ephi[(j0 + j) * GB] * tau_s[j0 + j];
+        for (int j = 0; j < 8; ++j) {
+          tj[j] = tau_s[j0 + j];
+          f[j] = ephi[(j0 + j) * GB] * tj[j];
+        }
         tmem_ld_wait();
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
@@ -447,6 +460,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
             for (int c = 0; c < NSL; ++c) x = x * 256 + acc[c][j];
             xd = (double)x;
           }
+          if (XOUT && j0 + j < wj) xg[(int64_t)(j0 + j) * GB] = xs * tj[j] * xd;  // X(g,n): 256 B per warp and column
           if (j & 1)
             rs2 = fma(f[j], xd, rs2);
           else
@@ -469,7 +483,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           const double sg = sigma[(int64_t)p * GB + g];
 #pragma unroll
           for (int q = 0; q < NSET - 1; ++q) rs += red[q * GB + g];
-          rho_s[(int64_t)p * GB + g] = 2.0 * sg * scalbn(rs, -8 * (NSL + 1));
+          rho_s[(int64_t)p * GB + g] = (XOUT ? 1.0 : 2.0) * sg * scalbn(rs, -8 * (NSL + 1));
         }
         asm volatile("bar.sync 1, %0;" ::"n"(32 * NEPI) : "memory");
         rs = 0.0;
@@ -528,7 +542,9 @@ static kldi_status tc_prepare(kldi_plan* P) {
   KLDI_CUDA(cudaMalloc(&P->d_chunk_off, sizeof(int64_t) * (P->n_blocks + 1)));
   KLDI_CUDA(cudaMemcpyAsync(P->d_chunk_off, h_chunk.data(), sizeof(int64_t) * (P->n_blocks + 1), cudaMemcpyHostToDevice, P->stream));
   KLDI_CUDA(cudaStreamSynchronize(P->stream));  // h_chunk goes out of scope
-  return ensure_smem_attr((const void*)tc::k_rho_i8<NSL>, tc::Cfg<NSL>::SMEM_BYTES, P->device);
+  kldi_status rc = ensure_smem_attr((const void*)tc::k_rho_i8<NSL, false>, tc::Cfg<NSL>::SMEM_BYTES, P->device);
+  if (rc != KLDI_OK) return rc;
+  return ensure_smem_attr((const void*)tc::k_rho_i8<NSL, true>, tc::Cfg<NSL>::SMEM_BYTES, P->device);
 }
 
 // Digit planes and row scales of one store of the rho layout (Phi or a gradient store), once per plan.
@@ -546,23 +562,28 @@ static kldi_status tc_prepare_store(kldi_plan* P, const double* store, unsigned 
   return KLDI_OK;
 }
 
-// The digits and column scales of D' (in P->d_Dp, triangular form), once per call.
+// The digits and column scales of the matrix in P->d_Dp, once per call: tri = D' (lower triangle, diagonal halved; only
+// that triangle of Dq is written, the rest stays zero) or the full D (the X builds of the nuclear gradient).
 template <int NSL>
-static kldi_status tc_slice_D(kldi_plan* P) {
+static kldi_status tc_slice_D(kldi_plan* P, bool tri = true) {
   const int n = P->n_ao;
+  if (tri && P->dq_upper_dirty)  // a full-D call has written the upper triangle: back to zero for the triangular form
+    KLDI_CUDA(cudaMemsetAsync(P->d_Dq, 0, sizeof(unsigned long long) * (size_t)n * n, P->stream));
+  P->dq_upper_dirty = !tri;
   double* cmax = P->d_tau + n;
   KLDI_CUDA(cudaMemsetAsync(cmax, 0, sizeof(double) * n, P->stream));
-  tc::k_colmax<<<dim3((n + 31) / 32, (n + 255) / 256), 256, 0, P->stream>>>(P->d_Dp, n, reinterpret_cast<unsigned long long*>(cmax));
+  tc::k_colmax<<<dim3((n + 31) / 32, (n + 255) / 256), 256, 0, P->stream>>>(P->d_Dp, n, reinterpret_cast<unsigned long long*>(cmax), tri ? 1 : 0);
   KLDI_LAUNCHED(P);
-  tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq);
+  tc::k_slice_D<NSL><<<dim3((n + 255) / 256, n), 256, 0, P->stream>>>(P->d_Dp, n, cmax, P->d_tau, P->d_Dq, tri ? 1 : 0);
   KLDI_LAUNCHED(P);
   return KLDI_OK;
 }
 
 // out_s[g] = 2 sum_{mu >= nu} D'_{mu,nu} A_{g,mu} A_{g,nu} for the store A (FP64 columns `store`, digit planes `planes`)
-template <int NSL>
+// XOUT: the full-D form, out_s[g] = sum_{mu,nu} D_{mu,nu} A_{g,mu} A_{g,nu} and x_out = A D (rho layout)
+template <int NSL, bool XOUT = false>
 static kldi_status tc_contract(kldi_plan* P, const double* store, const unsigned char* planes, const double* scales,
-                               double* out_s) {
+                               double* out_s, double* x_out = nullptr) {
   KLDI_CUDA(cudaMemsetAsync(out_s, 0, sizeof(double) * P->n_pad, P->stream));
   KLDI_CUDA(cudaMemsetAsync(P->d_ticket, 0, sizeof(int32_t) * 4, P->stream));
   const int grid = P->n_sm < P->n_tasks ? P->n_sm : P->n_tasks;
@@ -572,9 +593,9 @@ static kldi_status tc_contract(kldi_plan* P, const double* store, const unsigned
     KLDI_CUDA(cudaMalloc(&dbg, 32 * sizeof(long long)));
     KLDI_CUDA(cudaMemsetAsync(dbg, 0, 32 * sizeof(long long), P->stream));
   }
-  tc::k_rho_i8<NSL><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
+  tc::k_rho_i8<NSL, XOUT><<<grid, tc::NTHREADS, tc::Cfg<NSL>::SMEM_BYTES, P->stream>>>(
       P->d_tasks, P->n_tasks, P->d_ticket, P->d_kp, P->d_panel_off, P->d_chunk_off, P->d_colidx, store, planes, scales,
-      P->d_Dq, P->d_tau, P->n_ao, out_s, dbg);
+      P->d_Dq, P->d_tau, P->n_ao, out_s, x_out, dbg);
   KLDI_LAUNCHED(P);
   if (debug) {
     long long h[32];
@@ -624,6 +645,23 @@ kldi_status launch_tau_tc(kldi_plan* P) {
         KLDI_OK)
       return rc;
   return KLDI_OK;
+}
+
+// X = A D with the FULL D (already in P->d_Dp) for the store A = Phi (which = 0) or d_c Phi (which = 1 + c), written to
+// x_out in the rho layout; rho_out gets rowsum(A o X).  slice_d: split D into digits first (once per call).
+kldi_status launch_x_tc(kldi_plan* P, int which, double* x_out, double* rho_out, bool slice_d) {
+  kldi_status rc = tc_prepare<TC_NSL>(P);
+  if (rc != KLDI_OK) return rc;
+  const double* store = which == 0 ? P->d_phi : P->d_dphi[which - 1];
+  unsigned char** planes = which == 0 ? &P->d_phiq : &P->d_dphiq[which - 1];
+  double** scales = which == 0 ? &P->d_sigma : &P->d_dsigma[which - 1];
+  if ((rc = tc_prepare_store<TC_NSL>(P, store, planes, scales)) != KLDI_OK) return rc;
+  if (P->n_tasks == 0) {
+    KLDI_CUDA(cudaMemsetAsync(rho_out, 0, sizeof(double) * P->n_pad, P->stream));
+    return KLDI_OK;
+  }
+  if (slice_d && (rc = tc_slice_D<TC_NSL>(P, false)) != KLDI_OK) return rc;
+  return tc_contract<TC_NSL, true>(P, store, *planes, *scales, rho_out, x_out);
 }
 
 }  // namespace kldi

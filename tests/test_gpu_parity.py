@@ -431,6 +431,14 @@ def test_nuclear_gradient_parity(K, name, n):
     assert np.max(np.abs(ref)) > 1e-3
     assert np.max(np.abs(g - ref)) <= TOL_GRAD, np.max(np.abs(g - ref))
     assert abs(E - Eref) <= TOL_E
+    # KLDI_OPT_RHO_TC: the X build (full D) as int8 slice products on tcgen05, same bar; then back to the FP64 path
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)
+    Et, gt = plan.exc_grad(D)
+    assert np.max(np.abs(gt.cpu().numpy() - ref)) <= TOL_GRAD, np.max(np.abs(gt.cpu().numpy() - ref))
+    assert abs(Et - Eref) <= TOL_E
+    Et2, _ = plan.exc(D, K.KLDI_LDA_SLATER)           # triangular form right after a full-D digit split
+    assert abs(Et2 - Eref) <= TOL_E
+    plan.set_option(K.KLDI_OPT_RHO_TC, 0)
     # the same plan still serves the energy / potential path afterwards (the X store is an extra buffer)
     E2, _ = plan.exc(D, K.KLDI_LDA_SLATER)
     assert abs(E2 - Eref) <= TOL_E
@@ -460,6 +468,11 @@ def test_nuclear_gradient_gga_parity(K, name, n):
     assert g.shape == ref.shape == (wl.n_atoms, 3) and np.max(np.abs(ref)) > 1e-3
     assert np.max(np.abs(g - ref)) <= TOL_GRAD, np.max(np.abs(g - ref))
     assert abs(E - Eref) <= TOL_E
+    plan.set_option(K.KLDI_OPT_RHO_TC, 1)             # the three X^d builds on tcgen05
+    Et, gt = plan.exc_grad(D, K.KLDI_GGA_PBEX)
+    assert np.max(np.abs(gt.cpu().numpy() - ref)) <= TOL_GRAD, np.max(np.abs(gt.cpu().numpy() - ref))
+    assert abs(Et - Eref) <= TOL_E
+    plan.set_option(K.KLDI_OPT_RHO_TC, 0)
     E1, g1 = plan.exc_grad(D, K.KLDI_LDA_SLATER)
     ref1 = O.exc_nuclear_gradient_lda(basis_of(wl), wl.grid_xyz, wl.grid_w, wl.D)
     assert np.max(np.abs(g1.cpu().numpy() - ref1)) <= TOL_GRAD
