@@ -409,6 +409,19 @@ def main():
             if i >= 3:
                 tgg.append(plan_g.last_timings()["total"])
         grad_leg["gga_pbex_ms_per_call"] = float(np.median(tgg))
+        # the same calls with KLDI_OPT_RHO_TC (X builds / tau builds as int8 slice products on tcgen05)
+        plan_g.set_option(K.KLDI_OPT_RHO_TC, 1)
+        tc_ms = {}
+        for key, call in (("lda_slater", lambda: plan_g.exc_grad(D)), ("gga_pbex", lambda: plan_g.exc_grad(D, K.KLDI_GGA_PBEX)),
+                          ("eval_tau", lambda: plan_g.eval_tau(D))):
+            tt = []
+            for i in range(6):
+                call()
+                if i >= 2:
+                    tt.append(plan_g.last_timings()["total"])
+            tc_ms[key] = float(np.median(tt))
+        grad_leg["with_rho_tc_ms_per_call"] = tc_ms
+        plan_g.set_option(K.KLDI_OPT_RHO_TC, 0)
         # the meta-GGA contractions on the same plan (three LDA-form builds each)
         wv_t = torch.as_tensor(wl.grid_w, device="cuda").clone()
         Vt = torch.empty((wl.n_ao, wl.n_ao), dtype=torch.float64, device="cuda")
