@@ -436,12 +436,9 @@ __global__ void __launch_bounds__(NTHREADS, 1)
         int32_t acc[NSL][8];
 #pragma unroll
         for (int c = 0; c < NSL; ++c) tmem_ld8(tl + c * NT + j0, acc[c]);
-        double f[8], tj[8];  // tau_n Phi(g,n) of the columns j0 .. j0+7
+        double f[8];  // rho form: tau_n Phi(g,n) of the columns j0 .. j0+7; X form: tau_n alone (Phi is read when used)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          tj[j] = tau_s[j0 + j];
-          f[j] = ephi[(j0 + j) * GB] * tj[j];
-        }
+        for (int j = 0; j < 8; ++j) f[j] = tau_s[j0 + j];
         tmem_ld_wait();
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
@@ -460,11 +457,12 @@ __global__ void __launch_bounds__(NTHREADS, 1)
             for (int c = 0; c < NSL; ++c) x = x * 256 + acc[c][j];
             xd = (double)x;
           }
-          if (XOUT && j0 + j < wj) xg[(int64_t)(j0 + j) * GB] = xs * tj[j] * xd;  // X(g,n): 256 B per warp and column
+          const double t = f[j] * xd;
+          if (XOUT) xg[(int64_t)(j0 + j) * GB] = xs * t;  // X(g,n): 256 B per warp and column
           if (j & 1)
-            rs2 = fma(f[j], xd, rs2);
+            rs2 = fma(ephi[(j0 + j) * GB], t, rs2);
           else
-            rs = fma(f[j], xd, rs);
+            rs = fma(ephi[(j0 + j) * GB], t, rs);
         }
       }
       rs += rs2;
