@@ -260,15 +260,8 @@ __global__ void __launch_bounds__(NTHREADS, 1)
           __syncwarp();
           ++t;
         }
-        // the FP64 Phi columns of the tile for its epilogue (single buffer: wait for the previous epilogue); the columns
-        // of a panel are contiguous in the store, so this is ONE bulk copy
-        if (tile > 0) twait(1, b_eempty, (tile - 1) & 1);
-        if (lane == 0) {
-          const uint32_t bytes = (uint32_t)min(Wj, K8 - n0) * (GB * 8);
-          mbar_arrive_expect_tx(b_efull, bytes);
-          bulk_g2s(smem_u32(smem + C::OFF_EPI), phi + (base + n0) * GB, bytes, b_efull);
-        }
-        __syncwarp();
+        // (the tile's FP64 Phi columns for its epilogue are fetched by the epilogue warps themselves, see there: the
+        // producer never waits for an epilogue and keeps the ring full with the next tile's stages)
       }
     }
     for (int e = 0; e < NGRP; ++e) {  // one DONE stage per gather group (the other roles stop at the first)
@@ -416,6 +409,17 @@ __global__ void __launch_bounds__(NTHREADS, 1)
       const int p = hdr[4 * s + 0], n0 = hdr[4 * s + 1] & 0xffff, K8 = hdr[4 * s + 3];
       __syncwarp();
       if (lane == 0) mbar_arrive(b_empty + 8 * s);  // header read
+      if ((h2 & F_FIRST) && warp == W_EPI0) {
+        // first stage of a tile: fetch the tile's FP64 Phi columns for its epilogue (contiguous in the store: ONE bulk
+        // copy) as soon as every epilogue warp has left the previous tile (single buffer); it lands during the tile's MMAs
+        if (tile > 0) twait(4, b_eempty, (tile - 1) & 1);
+        if (lane == 0) {
+          const uint32_t bytes = (uint32_t)min((h2 >> 16) & 0xff, K8 - n0) * (GB * 8);
+          mbar_arrive_expect_tx(b_efull, bytes);
+          bulk_g2s(smem_u32(smem + C::OFF_EPI), phi + (panel_off[p] + n0) * GB, bytes, b_efull);
+        }
+        __syncwarp();
+      }
       if (!(h2 & F_LAST_TILE)) continue;
       const int wj = min((h2 >> 16) & 0xff, K8 - n0);  // real columns of the tile
       const volatile int* cn = cidx + ((h2 >> 24) & 3) * NT;
